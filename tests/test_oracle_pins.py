@@ -1,0 +1,299 @@
+"""Pins for the oracle — nothing here touches the CUDA path.
+
+Each test checks oracle/ against something the paper's statement of the problem or the
+mathematics fixes: closed forms, invariants, hand-evaluated special cases, dense brute force.
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import stag_inputs as si
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+RNG_SEED = 4242
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def load_spectra():
+    out = {}
+    with open(os.path.join(GOLDEN, "free_spectrum.txt")) as f:
+        for line in f:
+            if line.startswith("#"):
+                continue
+            Ls, rest = line.split("|")
+            L = tuple(int(v) for v in Ls.split())
+            out[L] = [(float(a.split(":")[0]), int(a.split(":")[1])) for a in rest.split(";")]
+    return out
+
+
+SPECTRA = load_spectra()
+
+
+# ---------------------------------------------------------------- P1 free-field spectrum
+@pytest.mark.parametrize("L", [(2, 2, 2, 2), (4, 4, 4, 4), (4, 4, 2, 6), (6, 4, 4, 2)])
+def test_P1_plane_waves_are_eigenvectors(L):
+    """D_eo D_oe v = -(sum_mu sin^2 p_mu) v for every momentum (north_star closed form)."""
+    U = si.links_unit(L)
+    colours = np.eye(3) + 0.25j
+    worst = 0.0
+    for k, n in enumerate(itertools.product(*[range(l) for l in L])):
+        v, p = si.source_plane_wave(L, n, colours[k % 3])
+        w = oracle.dslash_eo(L, U, oracle.dslash_oe(L, U, v))
+        lam = -np.sum(np.sin(p) ** 2)
+        worst = max(worst, np.linalg.norm(w - lam * v) / np.linalg.norm(v))
+    assert worst < 5e-15
+
+
+@pytest.mark.parametrize("L", [(2, 2, 2, 2), (4, 4, 4, 4), (4, 4, 2, 6)])
+def test_P1_full_spectrum_matches_golden(L):
+    """Whole multiset of eigenvalues of -D_eo D_oe (dense, mass 0) vs tests/golden."""
+    A = oracle.dense_A(L, si.links_unit(L), 0.0)
+    ev = np.linalg.eigvalsh(A)
+    expect = np.concatenate([[lam] * m for lam, m in SPECTRA[L]])
+    assert ev.size == expect.size == 3 * si.half_volume(L)
+    assert np.max(np.abs(np.sort(ev) - np.sort(expect))) < 1e-13
+
+
+def test_P1_phases_matter():
+    """With eta == 1 the spectrum differs: the golden file pins the anticommuting phases.
+    (Unit links, so dropping eta is the same as making every link +1 with eta -> 1; emulate
+    by feeding links that cancel eta: U_mu(x) = eta_mu(x) * 1 is still unitary, det = +-1.)"""
+    L = (4, 4, 4, 4)
+    x = si.site_coords(L)
+    U = si.links_unit(L)
+    cum = np.cumsum(x, axis=1)
+    for mu in range(1, 4):
+        U[:, mu] *= ((-1.0) ** cum[:, mu - 1])[:, None, None]
+    ev = np.linalg.eigvalsh(oracle.dense_A(L, U, 0.0))
+    distinct = np.unique(np.round(ev, 10))
+    assert distinct.size != 4  # golden 4^4 spectrum has exactly 4 distinct values
+
+
+# ---------------------------------------------------------------- P2 anti-hermiticity
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (6, 2, 4, 8), (2, 2, 2, 2)])
+def test_P2_antihermitian(L):
+    U = si.links_haar(L, 77)
+    psi = si.source_gaussian(L, 77, 1)
+    chi = si.source_gaussian(L, 77, 2)
+    lhs = np.vdot(chi, oracle.dslash_oe(L, U, psi))          # <chi_o, D_oe psi_e>
+    rhs = -np.vdot(oracle.dslash_eo(L, U, chi), psi)         # -<D_eo chi_o, psi_e>
+    assert abs(lhs - rhs) / abs(lhs) < 1e-14
+
+
+# ---------------------------------------------------------------- P3 gauge covariance
+@pytest.mark.parametrize("L,parity", [((4, 4, 4, 4), 0), ((4, 4, 4, 4), 1), ((6, 4, 2, 4), 1)])
+def test_P3_gauge_covariance(L, parity):
+    U = si.links_haar(L, 31)
+    g = si.gauge_transform_field(L, 31)
+    Ug = si.apply_gauge_transform(L, U, g)
+    psi = si.source_gaussian(L, 31, 3)
+    g_in = g[si.parity_sites(L, 1 - parity)]
+    g_out = g[si.parity_sites(L, parity)]
+    psi_g = np.einsum("xij,xj->xi", g_in, psi)
+    lhs = oracle.dslash(L, Ug, psi_g, parity)
+    rhs = np.einsum("xij,xj->xi", g_out, oracle.dslash(L, U, psi, parity))
+    assert rel(lhs, rhs) < 1e-14
+
+
+# ---------------------------------------------------------------- P4 Hermitian, bounded
+def test_P4_hermitian_positive_bounded():
+    L, m = (4, 4, 4, 4), 0.1
+    A = oracle.dense_A(L, si.links_haar(L, 5), m)
+    assert np.max(np.abs(A - A.conj().T)) < 1e-14
+    ev = np.linalg.eigvalsh(A)
+    assert ev.min() >= m * m - 1e-13
+    assert ev.max() <= m * m + 16.0
+    ev_free = np.linalg.eigvalsh(oracle.dense_A(L, si.links_unit(L), 0.0))
+    assert ev_free.min() >= -1e-13 and ev_free.max() <= 4.0 + 1e-13
+
+
+# ---------------------------------------------------------------- P5 delta source by hand
+@pytest.mark.parametrize("y", [(1, 2, 3, 0), (0, 0, 0, 0), (3, 1, 0, 3), (2, 3, 3, 3)])
+def test_P5_delta_source_by_hand(y):
+    """Unit links, delta at y (colour c): (D delta_y)(x) is
+         +1/2 eta_mu(x) s+  at x = y - mu   (forward hop from x reaches y)
+         -1/2 eta_mu(x) s-  at x = y + mu   (backward hop from x reaches y)
+       eta_0 = 1, eta_mu(x) = (-1)^(x0+..+x_{mu-1}); s = -1 when the hop crosses t = L3-1 -> 0."""
+    L = (4, 4, 4, 4)
+    U = si.links_unit(L)
+    py = sum(y) & 1
+    strides = np.array([1, L[0], L[0] * L[1], L[0] * L[1] * L[2]])
+    vh = si.half_volume(L)
+    c = 1
+    src = np.zeros((vh, 3), dtype=np.complex128)
+    src[int(np.dot(y, strides)) // 2, c] = 1.0
+    got = oracle.dslash(L, U, src, 1 - py)
+    expect = np.zeros_like(got)
+    for mu in range(4):
+        for sgn in (+1, -1):           # x = y - sgn*mu
+            x = list(y)
+            x[mu] = (y[mu] - sgn) % L[mu]
+            eta = 1.0 if mu == 0 else (-1.0) ** sum(x[:mu])
+            if sgn == +1:              # forward hop from x
+                s = -1.0 if (mu == 3 and x[3] == L[3] - 1) else 1.0
+                val = +0.5 * eta * s
+            else:                      # backward hop from x
+                s = -1.0 if (mu == 3 and x[3] == 0) else 1.0
+                val = -0.5 * eta * s
+            expect[int(np.dot(x, strides)) // 2, c] += val
+    assert np.max(np.abs(got - expect)) == 0.0
+    assert np.count_nonzero(got) == 8
+
+
+def test_dslash_vs_whole_lattice_roll_formulation():
+    """Consistency (not a pin): same operator written with np.roll on the full 4-d array."""
+    L = (4, 6, 2, 4)
+    U = si.links_haar(L, 9)
+    V = si.volume(L)
+    x = si.site_coords(L)
+    par = x.sum(axis=1) & 1
+    full = np.zeros((V, 3), dtype=np.complex128)
+    full[si.parity_sites(L, 0)] = si.source_gaussian(L, 9, 1)
+    full[si.parity_sites(L, 1)] = si.source_gaussian(L, 9, 2)
+    shp = (L[3], L[2], L[1], L[0])
+    psi = full.reshape(shp + (3,))
+    Ug = U.reshape(shp + (4, 3, 3))
+    xs = x.reshape(shp + (4,))
+    out = np.zeros_like(psi)
+    for mu in range(4):
+        ax = 3 - mu
+        eta = ((-1.0) ** xs[..., :mu].sum(axis=-1))[..., None]
+        sp = np.where((xs[..., mu] == L[mu] - 1) & (mu == 3), -1.0, 1.0)[..., None]
+        sm = np.where((xs[..., mu] == 0) & (mu == 3), -1.0, 1.0)[..., None]
+        fwd = np.einsum("...ij,...j->...i", Ug[..., mu, :, :], np.roll(psi, -1, axis=ax))
+        Ub = np.roll(Ug[..., mu, :, :], 1, axis=ax)
+        bwd = np.einsum("...ji,...j->...i", Ub.conj(), np.roll(psi, 1, axis=ax))
+        out += 0.5 * eta * (sp * fwd - sm * bwd)
+    out = out.reshape(V, 3)
+    for parity in (0, 1):
+        got = oracle.dslash(L, U, full[si.parity_sites(L, 1 - parity)], parity)
+        assert rel(got, out[si.parity_sites(L, parity)]) < 1e-15
+    assert par.sum() == V // 2
+
+
+# ---------------------------------------------------------------- P7 multi-shift CG
+SHIFTS = [0.01, 0.04, 0.16, 0.64]
+
+
+@pytest.mark.parametrize("L", [(2, 2, 2, 2), (4, 4, 4, 4)])
+def test_P7_dense_solves_every_shift(L):
+    m, stop = 0.1, 1e-10
+    U = si.links_haar(L, 1001)
+    b = si.source_gaussian(L, 1001, 1)
+    A = oracle.dense_A(L, U, m)
+    res = oracle.mshift_cg(L, U, b, m, SHIFTS, stop, 2000)
+    assert res["rc"] == 0
+    kappa = 16.0 / (m * m + min(SHIFTS))
+    for i, s in enumerate(SHIFTS):
+        xd = oracle.dense_solve(A, s, b)
+        xl = np.linalg.solve(A + s * np.eye(A.shape[0]), b.reshape(-1))   # library cross-check
+        assert rel(xd, xl) < 1e-12
+        assert rel(res["x"][i].reshape(-1), xd) < stop * kappa
+        true_res = b - oracle.apply_A(L, U, m, s, res["x"][i])
+        assert np.linalg.norm(true_res) / np.linalg.norm(b) <= stop      # (ii)
+
+
+def test_P7_unsorted_shifts_and_base_choice():
+    L, m = (4, 4, 4, 4), 0.1
+    U = si.links_haar(L, 1001)
+    b = si.source_gaussian(L, 1001, 1)
+    a = oracle.mshift_cg(L, U, b, m, SHIFTS, 1e-10, 2000)
+    perm = [2, 0, 3, 1]
+    c = oracle.mshift_cg(L, U, b, m, [SHIFTS[k] for k in perm], 1e-10, 2000)
+    assert a["iters"] == c["iters"]
+    for j, k in enumerate(perm):
+        assert rel(c["x"][j], a["x"][k]) < 1e-13
+
+
+def test_P7_shifted_residual_is_zeta_r_midrun():
+    """(iii) b - (A+sigma_i) x_i = zeta_i r at an intermediate iteration."""
+    L, m = (4, 4, 4, 4), 0.1
+    U = si.links_haar(L, 1001)
+    b = si.source_gaussian(L, 1001, 1)
+    for k in (1, 3, 17):
+        res = oracle.mshift_cg(L, U, b, m, SHIFTS, 1e-30, k)
+        assert res["rc"] == -5 and res["iters"] == k
+        assert res["zeta"][0] == 1.0
+        assert np.all(res["zeta"] > 0) and np.all(res["zeta"] <= 1.0)
+        for i, s in enumerate(SHIFTS):
+            true_res = b - oracle.apply_A(L, U, m, s, res["x"][i])
+            # rounding of b - (A+sigma)x is ~eps*||b||, so the scale of the check is ||b||
+            diff = np.linalg.norm(true_res - res["zeta"][i] * res["r"])
+            assert diff / np.linalg.norm(b) < 1e-14
+
+
+def test_P7_single_shift_is_textbook_cg():
+    """(iv) N = 1 equals textbook CG (Hestenes-Stiefel) iterate for iterate."""
+    L, m, s = (4, 4, 4, 4), 0.1, 0.04
+    U = si.links_haar(L, 1001)
+    b = si.source_gaussian(L, 1001, 1)
+    x = np.zeros_like(b)
+    r = b.copy()
+    p = b.copy()
+    rr = np.vdot(r, r).real
+    for k in range(1, 8):
+        q = oracle.apply_A(L, U, m, s, p)
+        al = rr / np.vdot(p, q).real
+        x = x + al * p
+        r = r - al * q
+        rr_new = np.vdot(r, r).real
+        p = r + (rr_new / rr) * p
+        rr = rr_new
+        got = oracle.mshift_cg(L, U, b, m, [s], 1e-30, k)
+        assert rel(got["x"][0], x) < 1e-13
+        assert rel(got["r"], r) < 1e-12
+
+
+def test_P7_finite_termination_free_field():
+    """(v) free 4^4: 4 distinct eigenvalues -> <= 4 iterations for every shift; free 2^4: 1."""
+    for L, kmax in (((4, 4, 4, 4), 4), ((2, 2, 2, 2), 1)):
+        U = si.links_unit(L)
+        b = si.source_gaussian(L, 3, 1)
+        res = oracle.mshift_cg(L, U, b, 0.1, SHIFTS, 1e-10, 50)
+        assert res["rc"] == 0 and res["iters"] <= kmax
+        for i, s in enumerate(SHIFTS):
+            tr = b - oracle.apply_A(L, U, 0.1, s, res["x"][i])
+            assert np.linalg.norm(tr) / np.linalg.norm(b) < 1e-13
+
+
+def test_P7_zero_source():
+    L = (4, 4, 4, 4)
+    U = si.links_haar(L, 1)
+    b = np.zeros((si.half_volume(L), 3), dtype=np.complex128)
+    res = oracle.mshift_cg(L, U, b, 0.1, SHIFTS, 1e-10, 50)
+    assert res["rc"] == 0 and res["iters"] == 0 and not res["x"].any()
+
+
+def test_P7_not_converged_and_bad_args():
+    L = (4, 4, 4, 4)
+    U = si.links_haar(L, 1)
+    b = si.source_gaussian(L, 1, 1)
+    assert oracle.mshift_cg(L, U, b, 0.1, SHIFTS, 1e-10, 3)["rc"] == -5
+    with pytest.raises(ValueError):
+        oracle.mshift_cg(L, U, b, 0.1, SHIFTS, -1.0, 3)
+    with pytest.raises(ValueError):
+        oracle.mshift_cg(L, U, b, 0.0, [0.0], 1e-10, 3)
+    with pytest.raises(ValueError):
+        oracle.dslash((4, 4, 3, 4), U[:192], b[:96], 0)
+
+
+# ---------------------------------------------------------------- P8 plane-wave closed form
+def test_P8_plane_wave_solution_and_partial_fraction():
+    L, m = (4, 4, 2, 6), 0.2
+    U = si.links_unit(L)
+    b, p = si.source_plane_wave(L, (1, 3, 0, 2), [1.0, 0.5j, -0.25])
+    lam = m * m + np.sum(np.sin(p) ** 2)
+    residues = [0.7, -0.2, 1.3, 0.05]
+    res = oracle.mshift_cg(L, U, b, m, SHIFTS, 1e-12, 10)
+    assert res["rc"] == 0 and res["iters"] == 1
+    for i, s in enumerate(SHIFTS):
+        assert rel(res["x"][i], b / (lam + s)) < 1e-14
+    y = oracle.partial_fraction(b, residues, 0.3, res["x"])
+    expect = b * (0.3 + sum(a / (lam + s) for a, s in zip(residues, SHIFTS)))
+    assert rel(y, expect) < 1e-14
