@@ -22,7 +22,8 @@
 //                          step): CG for shifted systems (ref
 //                          [9] = Jegerlehner hep-lat/9612014), zero start vector
 //                          (PAPER.md:129); recurrences as in DESIGN.md reading C4, in that
-//                          order and notation.  Pinned by P7, P8.
+//                          order and notation, zeta carried in ratio form (reading A15).
+//                          Pinned by P7, P8.
 //   * oracle_dense_*     — brute force for tiny lattices (north_star: "dense brute-force
 //                          linear solves on 2^4 and 4^4 lattices for every shift").
 //   * oracle_partial_fraction — y = residue0*b + sum_i residues[i]*x_i.
@@ -155,7 +156,14 @@ int oracle_mshift_cg(const int *L, const double *links, const double *b, double 
     std::vector<double> r(b, b + n), q(n), tmp(n);
     std::vector<std::vector<double> > p(nshift, std::vector<double>(b, b + n));
     std::memset(x, 0, sizeof(double) * n * nshift);
-    std::vector<double> zeta(nshift, 1.0), zeta_old(nshift, 1.0), zeta_new(nshift),
+    // theta_i = zeta_i / zetaold_i, carried as a state variable (reading A15): C4's
+    //   zetanew_i = zeta_i zetaold_i alphaold / (alpha betaold (zetaold_i - zeta_i)
+    //                                            + zetaold_i alphaold (1 + delta_i alpha))
+    // divided through by zetaold_i alphaold is
+    //   zetanew_i = zeta_i / ( (1 + delta_i alpha) + (alpha betaold / alphaold)(1 - theta_i) ),
+    // the same number, but without the product zeta_i*zetaold_i that underflows (-> 0/0 = NaN)
+    // for large shifts long before the base system converges.
+    std::vector<double> zeta(nshift, 1.0), theta(nshift, 1.0), theta_new(nshift),
         alpha_i(nshift), beta_i(nshift);
     double alpha_old = 1.0, beta_old = 0.0;
     const double bb = re_dot(b, b, n);
@@ -172,10 +180,9 @@ int oracle_mshift_cg(const int *L, const double *links, const double *b, double 
             const double alpha = rr / pq;
             if (!(pq > 0.0) || !std::isfinite(alpha)) { rc = -6; break; }
             for (int i = 0; i < nshift; ++i) {
-                zeta_new[i] = zeta[i] * zeta_old[i] * alpha_old /
-                              (alpha * beta_old * (zeta_old[i] - zeta[i]) +
-                               zeta_old[i] * alpha_old * (1.0 + delta[i] * alpha));
-                alpha_i[i] = alpha * zeta_new[i] / zeta[i];
+                theta_new[i] = 1.0 / ((1.0 + delta[i] * alpha) +
+                                      (alpha * beta_old / alpha_old) * (1.0 - theta[i]));
+                alpha_i[i] = alpha * theta_new[i];          // alpha zetanew_i / zeta_i
             }
             for (int i = 0; i < nshift; ++i) {
                 double *xi = x + (long)i * n;
@@ -188,17 +195,16 @@ int oracle_mshift_cg(const int *L, const double *links, const double *b, double 
             const double rr_new = re_dot(r.data(), r.data(), n);
             const double beta = rr_new / rr;
             for (int i = 0; i < nshift; ++i) {
-                const double ratio = zeta_new[i] / zeta[i];
-                beta_i[i] = beta * ratio * ratio;
+                beta_i[i] = beta * theta_new[i] * theta_new[i];   // beta (zetanew_i / zeta_i)^2
             }
             for (int i = 0; i < nshift; ++i) {
                 double *pi = p[i].data();
-                const double zn = zeta_new[i], bi = beta_i[i];
+                const double zn = zeta[i] * theta_new[i], bi = beta_i[i];   // zetanew_i
                 const double *rp = r.data();
 #pragma omp parallel for num_threads(g_threads) schedule(static)
                 for (long k = 0; k < n; ++k) pi[k] = zn * rp[k] + bi * pi[k];
             }
-            for (int i = 0; i < nshift; ++i) { zeta_old[i] = zeta[i]; zeta[i] = zeta_new[i]; }
+            for (int i = 0; i < nshift; ++i) { zeta[i] *= theta_new[i]; theta[i] = theta_new[i]; }
             alpha_old = alpha; beta_old = beta; rr = rr_new;
             iters = it;
             if (rr_hist) rr_hist[it] = rr;

@@ -199,6 +199,26 @@ def test_P7_dense_solves_every_shift(L):
         assert np.linalg.norm(true_res) / np.linalg.norm(b) <= stop      # (ii)
 
 
+def test_P7_wide_shift_range_no_underflow():
+    """Config-4-like shifts (1e-5..20) on 4^4: zeta_i of the large shifts underflows long before
+    the base system converges (~600 iterations); every x_i must still be the dense solution
+    (reading A15: the zeta recurrence is carried in ratio form, no 0/0)."""
+    L, m, stop = (4, 4, 4, 4), 0.01, 1e-10
+    shifts = [1e-5 * (2e6) ** (i / 15) for i in range(16)]
+    U = si.links_haar(L, 1004)
+    b = si.source_gaussian(L, 1004, 1)
+    A = oracle.dense_A(L, U, m)
+    res = oracle.mshift_cg(L, U, b, m, shifts, stop, 5000)
+    assert res["rc"] == 0 and res["iters"] > 300
+    assert np.all(np.isfinite(res["x"])) and np.all(np.isfinite(res["zeta"]))
+    assert res["zeta"][-1] < 1e-200
+    for i, s in enumerate(shifts):
+        xd = oracle.dense_solve(A, s, b)
+        assert rel(res["x"][i].reshape(-1), xd) < stop * 16.0 / (m * m + s)
+        tr = b - oracle.apply_A(L, U, m, s, res["x"][i])
+        assert np.linalg.norm(tr) / np.linalg.norm(b) <= stop
+
+
 def test_P7_unsorted_shifts_and_base_choice():
     L, m = (4, 4, 4, 4), 0.1
     U = si.links_haar(L, 1001)
