@@ -1,0 +1,167 @@
+/* stag.h — C ABI of the B200-native staggered Dslash + multi-shift CG library.
+ *
+ * The data-parallel hot path of the RHMC of arxiv 1010.5433 ("Staggered fermions
+ * simulations on GPUs", Bonati, Cossu, D'Elia, Di Giacomo): the even/odd-preconditioned
+ * staggered hopping term D_eo / D_oe (PAPER.md:45 "even/odd preconditioning", :87 "Dirac
+ * kernel") applied inside the multi-shift conjugate-gradient solve of
+ *
+ *        (m^2 - D_eo D_oe + sigma_i) x_i = b,     i = 0 .. nshift-1,
+ *
+ * the solve the rational approximation needs for MD forces and for the Metropolis step
+ * (PAPER.md:43, :49).  The paper has no API (one monolithic program); the entry
+ * points are the ones BASELINE.json:north_star names and their arguments are the paper's
+ * statement of the problem: lattice extents, links, mass, shifts and residues, stopping
+ * residual.  Definitions the paper leaves out (normalisation, phases, boundary condition)
+ * are the readings A1-A5 in DESIGN.md.
+ *
+ * Operator (reading A1-A5).  Site x = (x0,x1,x2,x3), x3 = time, parity
+ * (x0+x1+x2+x3) & 1 (0 = even), U_mu(x) in SU(3) the link from x to x+mu:
+ *
+ *   (D psi)(x) = 1/2 sum_mu eta_mu(x) [ s+ U_mu(x) psi(x+mu) - s- U_mu(x-mu)^dagger psi(x-mu) ]
+ *   eta_0 = 1, eta_mu(x) = (-1)^(x0+...+x_{mu-1});   antiperiodic time: s+ = -1 iff mu = 3 and
+ *   x3 = L3-1, s- = -1 iff mu = 3 and x3 = 0; periodic in 0,1,2.
+ *   D_eo: even output from odd input.  D_oe: odd output from even input.
+ *
+ * CONVENTIONS
+ *   Pointers   "host_*" arguments are host pointers, everything else named dev_* / packed /
+ *              workspace / *_even / *_odd is a DEVICE pointer.  The caller owns every buffer
+ *              (e.g. torch tensors' data_ptr()); the library allocates nothing per call.  A
+ *              stag_ctx owns only the geometry and a few bytes of pinned host memory.
+ *   stream     a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   Errors     every int-returning function returns STAG_OK (0) or a negative STAG_ERR_*;
+ *              no exceptions, no exit().  Kernel launches are asynchronous: a launch error
+ *              shows up as STAG_ERR_CUDA from the same or a later call.
+ *   Aliasing   input and output buffers of one call must not overlap.
+ *   Threads    a stag_ctx may be shared by calls on different streams, except that only one
+ *              stag_mshift_cg* call may be in flight per ctx at a time.
+ *
+ * CANONICAL (interchange) FORMATS — always fp64
+ *   site index   lex(x) = x0 + L0*(x1 + L1*(x2 + L2*x3));  one-parity index e = lex(x)/2
+ *   links        double [V][4][3][3][2]   (site lex, direction mu, row, column, re/im), raw
+ *                SU(3): no 1/2, no eta, no boundary sign — the library applies them.
+ *   vector       double [Vh][3][2]        (e, colour, re/im) on one parity, Vh = V/2.
+ *
+ * DEVICE (compute) FORMATS — private to the library, sizes from the *_bytes() functions
+ *   packed gauge "hopping matrices", per output parity p, direction d = 2*mu + (0 fwd | 1 bwd):
+ *                W_d(x) = +1/2 eta s+ U_mu(x)  or  -1/2 eta s- U_mu(x-mu)^dagger,  indexed by
+ *                the OUTPUT site e, stored as planes of 16-byte chunks [p][d][chunk][e] so that
+ *                every load is a coalesced, aligned 128-bit access.  recon = 18 keeps all three
+ *                rows, recon = 12 keeps rows 1-2 and rebuilds row 3.
+ *   vector       colour planes of 16-byte chunks [chunk][e]: fp64 = 3 planes of one complex;
+ *                fp32 = one plane of (c0,c1) + one 8-byte plane of c2.  Convert with
+ *                stag_vector_pack / stag_vector_unpack.
+ */
+#ifndef STAG_H_
+#define STAG_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define STAG_MAX_SHIFTS 32
+
+enum {
+    STAG_OK = 0,
+    STAG_ERR_BADARG = -1,       /* odd / too small extent, bad enum, null pointer, bad shift ... */
+    STAG_ERR_UNSUPPORTED = -2,  /* valid request this build cannot serve (e.g. V >= 2^31)      */
+    STAG_ERR_CUDA = -3,         /* a CUDA runtime call or kernel launch failed                  */
+    STAG_ERR_NOT_SU3 = -4,      /* recon = 12 asked for links that are not SU(3) to 1e-12       */
+    STAG_ERR_NOTCONV = -5,      /* maxiter reached (or fp32 stagnation); outputs still written  */
+    STAG_ERR_BREAKDOWN = -6     /* <p,Ap> <= 0 or NaN inside CG                                 */
+};
+enum { STAG_F64 = 0, STAG_F32 = 1 };
+enum { STAG_RECON18 = 18, STAG_RECON12 = 12 };
+
+typedef struct stag_ctx stag_ctx;
+
+/* Result of one multi-shift solve (host struct, filled after the final stream sync). */
+typedef struct stag_cg_info {
+    int iters;                             /* iterations of the base (smallest-shift) system   */
+    int converged;                         /* 1 iff ||r||/||b|| <= stop was reached            */
+    int breakdown;                         /* 1 iff <p,Ap> <= 0 or NaN                         */
+    int stagnated;                         /* fp32 only: stopped because ||r|| stopped falling */
+    double bnorm2;                         /* <b,b>                                            */
+    double rnorm2;                         /* iterated <r,r> of the base system at exit        */
+    double resid_iter[STAG_MAX_SHIFTS];    /* iterated zeta_i*||r||/||b|| per shift at exit/freeze */
+    int iters_shift[STAG_MAX_SHIFTS];      /* iteration at which shift i stopped being updated */
+} stag_cg_info;
+
+/* ---- context --------------------------------------------------------------------------- */
+/* L[mu] even and >= 2, time = L[3]; V = L0*L1*L2*L3 must be < 2^31.  Uses the current CUDA
+ * device.  *out is set on success only. */
+int stag_ctx_create(const int L[4], stag_ctx **out);
+void stag_ctx_destroy(stag_ctx *ctx);
+const char *stag_strerror(int err);
+/* Tuning knobs (integers): "dslash_block" (threads per CTA: 64|128|256), "cg_check_every"
+ * (iterations between convergence polls), "cg_graph" (0|1: replay iterations as a CUDA
+ * graph), "cg_freeze" (0|1: stop updating converged shifts, reading A10). */
+int stag_set_option(stag_ctx *ctx, const char *key, int value);
+int stag_get_option(const stag_ctx *ctx, const char *key, int *value);
+
+/* ---- sizes (bytes) --------------------------------------------------------------------- */
+size_t stag_gauge_canonical_bytes(const stag_ctx *ctx);              /* 4*V*18 doubles     */
+size_t stag_gauge_packed_bytes(const stag_ctx *ctx, int prec, int recon);
+size_t stag_vector_canonical_bytes(const stag_ctx *ctx);             /* Vh*6 doubles       */
+size_t stag_vector_bytes(const stag_ctx *ctx, int prec);             /* device format      */
+size_t stag_cg_workspace_bytes(const stag_ctx *ctx, int prec, int nshift);
+size_t stag_host_scratch_bytes(const stag_ctx *ctx, int prec, int nshift); /* for *_host calls */
+
+/* ---- a1: gauge load + pack (setup; "copy the starting gauge configuration on the
+ *      device memory at the beginning", :109 12-real storage, :113 float cast, :119 layout) --- */
+/* H->D copy of canonical links, asynchronous on stream (pin host_links for true overlap). */
+int stag_gauge_load(const stag_ctx *ctx, const double *host_links,
+                    double *dev_links_canonical, void *stream);
+/* canonical device links -> packed hopping matrices.  prec = STAG_F32 rounds to nearest
+ * (b = (float)a).  recon = 12 first checks max|U U^dag - 1| <= 1e-12 and
+ * |det U - 1| <= 1e-12 on the device and returns STAG_ERR_NOT_SU3 otherwise (synchronises
+ * the stream; recon = 18 does not synchronise). */
+int stag_gauge_pack(const stag_ctx *ctx, const double *dev_links_canonical,
+                    void *dev_packed, int prec, int recon, void *stream);
+
+/* ---- vector format conversion (device to device, asynchronous) --------------------------- */
+int stag_vector_pack(const stag_ctx *ctx, const double *dev_canonical, void *dev_vec,
+                     int prec, void *stream);
+int stag_vector_unpack(const stag_ctx *ctx, const void *dev_vec, int prec,
+                       double *dev_canonical, void *stream);
+
+/* ---- a2/a3: the hopping term (570 flop/site).  One kernel launch, no sync. ---- */
+int stag_dslash_eo(const stag_ctx *ctx, const void *packed, int prec, int recon,
+                   const void *in_odd, void *out_even, void *stream);
+int stag_dslash_oe(const stag_ctx *ctx, const void *packed, int prec, int recon,
+                   const void *in_even, void *out_odd, void *stream);
+
+/* ---- a3-a7: multi-shift CG (ref [9]); start vector zero for every shift.
+ *   b_even     source, device format
+ *   shifts     host, nshift values sigma_i >= 0, any order; 1 <= nshift <= STAG_MAX_SHIFTS
+ *   residues   host, nullable; with y_even != NULL:  y = residue0*b + sum_i residues[i]*x_i
+ *   stop       on the iterated ||r||/||b|| of the smallest-shift system, tested every iteration
+ *   x_even     out, nshift contiguous device-format vectors (x_i at byte offset
+ *              i*stag_vector_bytes)
+ *   workspace  stag_cg_workspace_bytes(ctx, prec, nshift) bytes, 256-byte aligned
+ *   info       host, nullable
+ * Vectors are prec; every reduction and scalar recurrence is fp64.  Synchronises the stream
+ * before returning.  STAG_ERR_NOTCONV / STAG_ERR_BREAKDOWN still write x (and y) and info. */
+int stag_mshift_cg(const stag_ctx *ctx, const void *packed, int prec, int recon,
+                   const void *b_even, double mass, int nshift, const double *host_shifts,
+                   const double *host_residues, double residue0, double stop, int maxiter,
+                   void *x_even, void *y_even, void *workspace, stag_cg_info *info,
+                   void *stream);
+
+/* ---- the same calls on HOST buffers in canonical fp64 format (copies inside) --------------
+ * dev_scratch: stag_host_scratch_bytes(ctx, prec, nshift) bytes of device memory
+ * (nshift = 0 for stag_dslash_host).  out_parity: 0 = D_eo, 1 = D_oe. */
+int stag_dslash_host(const stag_ctx *ctx, const void *packed, int prec, int recon,
+                     int out_parity, const double *host_in, double *host_out,
+                     void *dev_scratch, void *stream);
+int stag_mshift_cg_host(const stag_ctx *ctx, const void *packed, int prec, int recon,
+                        const double *host_b, double mass, int nshift,
+                        const double *host_shifts, const double *host_residues,
+                        double residue0, double stop, int maxiter, double *host_x,
+                        double *host_y, void *dev_scratch, stag_cg_info *info, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STAG_H_ */

@@ -1,0 +1,169 @@
+// stag_common.cuh — geometry, context and small device helpers shared by the kernels of
+// libstag_b200.so (sm_100a).  Private to the CUDA path; the oracle includes none of this.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/stag.h"
+
+namespace stag {
+
+// ---- exact unsigned division by a runtime constant (n < 2^31) ------------------------------
+struct FastDiv {
+    uint32_t d, mul, shift;
+    __host__ void init(uint32_t div) {
+        d = div;
+        shift = 0;
+        while ((1u << shift) < div) ++shift;
+        mul = (uint32_t)((((uint64_t)1 << (32 + shift)) + div - 1) / div - ((uint64_t)1 << 32));
+    }
+    __device__ __forceinline__ uint32_t div(uint32_t n) const {
+        return (__umulhi(n, mul) + n) >> shift;
+    }
+};
+
+// ---- lattice geometry, passed by value to every kernel ---------------------------------------
+struct Geom {
+    int L[4];
+    int Lh0;      // L0 / 2: sites of one parity per x0-row
+    int Vh;       // sites per parity
+    int V;
+    FastDiv dLh0, dL1, dL2;
+};
+
+// coordinates of the site with one-parity index e and parity par
+struct Site {
+    int x0, x1, x2, x3;
+    int lex;
+};
+
+__device__ __forceinline__ Site site_of(const Geom &g, int e, int par) {
+    Site s;
+    const uint32_t row = g.dLh0.div((uint32_t)e);            // x1 + L1*(x2 + L2*x3)
+    const int h = e - (int)row * g.Lh0;
+    const uint32_t r2 = g.dL1.div(row);
+    s.x1 = (int)row - (int)r2 * g.L[1];
+    s.x3 = (int)g.dL2.div(r2);
+    s.x2 = (int)r2 - s.x3 * g.L[2];
+    s.x0 = 2 * h + ((s.x1 + s.x2 + s.x3 + par) & 1);
+    s.lex = s.x0 + g.L[0] * (int)row;
+    return s;
+}
+
+// ---- context -------------------------------------------------------------------------------
+struct Options {
+    int dslash_block;        // threads per CTA of the Dslash kernels: 64 | 128 | 256
+    int dslash_ctas_per_sm;  // 0: one CTA per block of sites; k > 0: persistent grid of k*SMs CTAs
+    int cg_check_every;      // iterations between convergence polls (= iterations per CUDA graph)
+    int cg_graph;            // replay the iteration batch as a CUDA graph
+    int cg_freeze;           // stop updating converged shifts (reading A10)
+    int cg_ctas_per_sm;      // persistent grid size of the CG streaming kernels, per SM
+};
+
+}  // namespace stag
+
+struct stag_ctx {
+    stag::Geom g;
+    stag::Options opt;
+    int device;
+    int num_sms;
+    int *pinned_flags;   // small pinned (mapped) host buffer: status words, convergence polls
+    void *pinned_info;   // pinned staging for the CG state upload / read-back (one CgState)
+};
+
+namespace stag {
+
+#define STAG_CUDA_OK(call)                                  \
+    do {                                                    \
+        cudaError_t e__ = (call);                           \
+        if (e__ != cudaSuccess) return STAG_ERR_CUDA;       \
+    } while (0)
+
+inline bool valid_prec(int p) { return p == STAG_F64 || p == STAG_F32; }
+inline bool valid_recon(int r) { return r == STAG_RECON18 || r == STAG_RECON12; }
+
+// bytes of one link set plane group: (recon reals) * sizeof(T) per site
+inline size_t link_bytes_per_site(int prec, int recon) {
+    return (size_t)recon * (prec == STAG_F64 ? 8 : 4);
+}
+inline size_t vec_bytes_per_site(int prec) { return (size_t)6 * (prec == STAG_F64 ? 8 : 4); }
+inline size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
+
+// ---- streaming / cached 128-bit and 64-bit loads ---------------------------------------------
+// Links are read exactly once per Dslash: keep them out of L1 and first in line for L2
+// eviction so that the (re-used) colour vectors stay cached.
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t pol;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ double2 ld_stream(const double2 *p, uint64_t pol) {
+    double2 r;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
+        : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ float4 ld_stream(const float4 *p, uint64_t pol) {
+    float4 r;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+        : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p), "l"(pol));
+    return r;
+}
+__device__ __forceinline__ float2 ld_stream(const float2 *p, uint64_t pol) {
+    float2 r;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;"
+        : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(pol));
+    return r;
+}
+// Neighbour colour vectors are re-used by up to 8 output sites: read-only path, L1-allocating.
+__device__ __forceinline__ double2 ld_reuse(const double2 *p) { return __ldg(p); }
+__device__ __forceinline__ float4 ld_reuse(const float4 *p) { return __ldg(p); }
+__device__ __forceinline__ float2 ld_reuse(const float2 *p) { return __ldg(p); }
+
+// ---- block-wide sum of one double (deterministic for a fixed block size) ----------------------
+template <int BLOCK>
+__device__ __forceinline__ double block_sum(double v, double *smem /* BLOCK/32 doubles */) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) smem[warp] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (warp == 0) {
+        s = lane < BLOCK / 32 ? smem[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    }
+    return s;  // valid in warp 0 (all its lanes)
+}
+
+// ---- grid-wide sum, finished by the last CTA to arrive ------------------------------------------
+// Every CTA writes its partial to partials[blockIdx.x]; the CTA that draws the last ticket adds
+// all partials in index order (deterministic for a fixed grid) and gets `true` with the total in
+// every lane of its warp 0.  One __threadfence per CTA, at its very end (a gpu-scope fence
+// invalidates L1, so the kernels that use this are persistent: many tiles, one fence).
+template <int BLOCK>
+__device__ __forceinline__ bool grid_sum_last_cta(double v, double *partials, unsigned int *ticket,
+                                                  double *smem /* BLOCK/32 + 1 doubles */,
+                                                  double &total) {
+    const double s = block_sum<BLOCK>(v, smem);
+    int *flag = reinterpret_cast<int *>(smem + BLOCK / 32);
+    if (threadIdx.x == 0) {
+        __stcg(partials + blockIdx.x, s);
+        __threadfence();
+        const unsigned int t = atomicAdd(ticket, 1u);
+        *flag = (t == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!*flag) return false;
+    __threadfence();
+    double t = 0.0;
+    for (unsigned int i = threadIdx.x; i < gridDim.x; i += BLOCK) t += __ldcg(partials + i);
+    total = block_sum<BLOCK>(t, smem);
+    if (threadIdx.x == 0) *ticket = 0u;
+    return true;
+}
+
+}  // namespace stag

@@ -1,0 +1,125 @@
+// stag_ctx.cu — context, options, sizes, error strings of libstag_b200.so.
+#include <cstring>
+#include <new>
+
+#include "stag_cg.cuh"
+
+using namespace stag;
+
+extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
+    if (!L || !out) return STAG_ERR_BADARG;
+    long long V = 1;
+    for (int mu = 0; mu < 4; ++mu) {
+        if (L[mu] < 2 || (L[mu] & 1)) return STAG_ERR_BADARG;
+        V *= L[mu];
+        if (V >= (1ll << 31)) return STAG_ERR_UNSUPPORTED;
+    }
+    stag_ctx *c = new (std::nothrow) stag_ctx;
+    if (!c) return STAG_ERR_CUDA;
+    std::memset(c, 0, sizeof(*c));
+    Geom &g = c->g;
+    for (int mu = 0; mu < 4; ++mu) g.L[mu] = L[mu];
+    g.Lh0 = L[0] / 2;
+    g.V = (int)V;
+    g.Vh = (int)(V / 2);
+    g.dLh0.init((uint32_t)g.Lh0);
+    g.dL1.init((uint32_t)L[1]);
+    g.dL2.init((uint32_t)L[2]);
+    c->opt.dslash_block = 128;
+    c->opt.dslash_ctas_per_sm = 0;   // 0 = one CTA per 'dslash_block' sites (non-persistent)
+    c->opt.cg_check_every = 16;
+    c->opt.cg_graph = 1;
+    c->opt.cg_freeze = 1;
+    c->opt.cg_ctas_per_sm = 8;
+    if (cudaGetDevice(&c->device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess ||
+        cudaHostAlloc((void **)&c->pinned_flags, 64, cudaHostAllocMapped) != cudaSuccess ||
+        cudaHostAlloc(&c->pinned_info, sizeof(CgState), cudaHostAllocDefault) != cudaSuccess) {
+        cudaGetLastError();
+        stag_ctx_destroy(c);
+        return STAG_ERR_CUDA;
+    }
+    *out = c;
+    return STAG_OK;
+}
+
+extern "C" void stag_ctx_destroy(stag_ctx *ctx) {
+    if (!ctx) return;
+    if (ctx->pinned_flags) cudaFreeHost(ctx->pinned_flags);
+    if (ctx->pinned_info) cudaFreeHost(ctx->pinned_info);
+    delete ctx;
+}
+
+extern "C" const char *stag_strerror(int err) {
+    switch (err) {
+        case STAG_OK: return "ok";
+        case STAG_ERR_BADARG: return "bad argument";
+        case STAG_ERR_UNSUPPORTED: return "unsupported request";
+        case STAG_ERR_CUDA: return "CUDA runtime error";
+        case STAG_ERR_NOT_SU3: return "links are not SU(3): 12-real reconstruction impossible";
+        case STAG_ERR_NOTCONV: return "multi-shift CG did not converge";
+        case STAG_ERR_BREAKDOWN: return "multi-shift CG breakdown (<p,Ap> <= 0 or NaN)";
+        default: return "unknown error";
+    }
+}
+
+static int *option_slot(Options &o, const char *key) {
+    if (!key) return nullptr;
+    if (!std::strcmp(key, "dslash_block")) return &o.dslash_block;
+    if (!std::strcmp(key, "dslash_ctas_per_sm")) return &o.dslash_ctas_per_sm;
+    if (!std::strcmp(key, "cg_check_every")) return &o.cg_check_every;
+    if (!std::strcmp(key, "cg_graph")) return &o.cg_graph;
+    if (!std::strcmp(key, "cg_freeze")) return &o.cg_freeze;
+    if (!std::strcmp(key, "cg_ctas_per_sm")) return &o.cg_ctas_per_sm;
+    return nullptr;
+}
+
+extern "C" int stag_set_option(stag_ctx *ctx, const char *key, int value) {
+    if (!ctx) return STAG_ERR_BADARG;
+    int *slot = option_slot(ctx->opt, key);
+    if (!slot) return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.dslash_block && value != 64 && value != 128 && value != 256)
+        return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.cg_check_every && value < 1) return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.cg_ctas_per_sm && (value < 1 || value > 16)) return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.dslash_ctas_per_sm && (value < 0 || value > 32)) return STAG_ERR_BADARG;
+    *slot = value;
+    return STAG_OK;
+}
+
+extern "C" int stag_get_option(const stag_ctx *ctx, const char *key, int *value) {
+    if (!ctx || !value) return STAG_ERR_BADARG;
+    int *slot = option_slot(const_cast<stag_ctx *>(ctx)->opt, key);
+    if (!slot) return STAG_ERR_BADARG;
+    *value = *slot;
+    return STAG_OK;
+}
+
+// ---- sizes ------------------------------------------------------------------------------------
+extern "C" size_t stag_gauge_canonical_bytes(const stag_ctx *ctx) {
+    return ctx ? (size_t)ctx->g.V * 4 * 18 * sizeof(double) : 0;
+}
+extern "C" size_t stag_gauge_packed_bytes(const stag_ctx *ctx, int prec, int recon) {
+    if (!ctx || !valid_prec(prec) || !valid_recon(recon)) return 0;
+    return (size_t)16 * ctx->g.Vh * link_bytes_per_site(prec, recon);   // 2 parities x 8 directions
+}
+extern "C" size_t stag_vector_canonical_bytes(const stag_ctx *ctx) {
+    return ctx ? (size_t)ctx->g.Vh * 6 * sizeof(double) : 0;
+}
+extern "C" size_t stag_vector_bytes(const stag_ctx *ctx, int prec) {
+    if (!ctx || !valid_prec(prec)) return 0;
+    return (size_t)ctx->g.Vh * vec_bytes_per_site(prec);
+}
+extern "C" size_t stag_cg_workspace_bytes(const stag_ctx *ctx, int prec, int nshift) {
+    if (!ctx || !valid_prec(prec) || nshift < 1 || nshift > STAG_MAX_SHIFTS) return 0;
+    return cg_workspace_layout(ctx, prec, nshift, nullptr);
+}
+extern "C" size_t stag_host_scratch_bytes(const stag_ctx *ctx, int prec, int nshift) {
+    if (!ctx || !valid_prec(prec) || nshift < 0 || nshift > STAG_MAX_SHIFTS) return 0;
+    const size_t canon = align256(stag_vector_canonical_bytes(ctx));
+    const size_t vec = align256(stag_vector_bytes(ctx, prec));
+    if (nshift == 0) return canon + 2 * vec;                       // canonical staging, in, out
+    // canonical staging, b, y, x[nshift], CG workspace
+    return canon + 2 * vec + align256((size_t)nshift * stag_vector_bytes(ctx, prec)) +
+           align256(cg_workspace_layout(ctx, prec, nshift, nullptr));
+}

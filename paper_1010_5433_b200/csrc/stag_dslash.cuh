@@ -1,0 +1,157 @@
+// stag_dslash.cuh — the per-site body of the staggered hopping term ("a
+// different thread is associated to every (even) site").
+//
+//   (D psi)(x) = sum_{d=0..7} W_d(x) psi(nbr_d(x)),   d = 2*mu (forward) | 2*mu+1 (backward)
+//
+// with the hopping matrices W_d packed by stag_gauge_pack (1/2, eta, boundary sign, the
+// dagger and the minus of the backward term are already folded in).  8 x (3x3 complex
+// mat-vec) + 7 vector adds = 570 flop / site (BASELINE.json:north_star).  Not a dense
+// contraction (a different matrix per site and direction): CUDA cores, no tensor cores.
+//
+// Memory behaviour: every thread streams its 8 hopping matrices with aligned, fully
+// coalesced 128-bit loads that bypass L1 and are marked evict-first in L2 (read exactly once
+// per Dslash); the 8 neighbour colour vectors come through the read-only L1/L2 path, where
+// the up-to-8-fold re-use between neighbouring sites is served.
+#pragma once
+
+#include "stag_common.cuh"
+
+namespace stag {
+
+template <typename T> struct Prec;
+template <> struct Prec<double> {
+    static constexpr int id = STAG_F64;
+    static constexpr int vec_chunks = 3;   // full 16-byte chunks per colour vector
+};
+template <> struct Prec<float> {
+    static constexpr int id = STAG_F32;
+    static constexpr int vec_chunks = 1;   // + one 8-byte tail chunk
+};
+
+// ---- colour-vector load / store in the device format ----------------------------------------
+__device__ __forceinline__ void load_vec(const char *__restrict__ v, int Vh, int e, double (&x)[6]) {
+    const double2 *p = reinterpret_cast<const double2 *>(v) + e;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double2 t = ld_reuse(p + (size_t)c * Vh);
+        x[2 * c] = t.x; x[2 * c + 1] = t.y;
+    }
+}
+__device__ __forceinline__ void load_vec(const char *__restrict__ v, int Vh, int e, float (&x)[6]) {
+    const float4 a = ld_reuse(reinterpret_cast<const float4 *>(v) + e);
+    const float2 b = ld_reuse(reinterpret_cast<const float2 *>(v + (size_t)Vh * 16) + e);
+    x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = b.x; x[5] = b.y;
+}
+__device__ __forceinline__ void store_vec(char *__restrict__ v, int Vh, int e, const double (&x)[6]) {
+    double2 *p = reinterpret_cast<double2 *>(v) + e;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) p[(size_t)c * Vh] = make_double2(x[2 * c], x[2 * c + 1]);
+}
+__device__ __forceinline__ void store_vec(char *__restrict__ v, int Vh, int e, const float (&x)[6]) {
+    reinterpret_cast<float4 *>(v)[e] = make_float4(x[0], x[1], x[2], x[3]);
+    reinterpret_cast<float2 *>(v + (size_t)Vh * 16)[e] = make_float2(x[4], x[5]);
+}
+
+// ---- hopping-matrix load: u[18] = row-major 3x3 complex (re,im interleaved) -------------------
+// c3: factor of the rebuilt third row (recon 12 only).  Rows 1-2 carry the folded factor
+// f = +-1/2, so conj(row1 x row2) = f^2 * row3_true = (1/4) row3_true and the stored matrix
+// needs f * row3_true = (4f) * conj(row1 x row2):  c3 = 4f = +-2  (reading A6).
+template <typename T>
+__device__ __forceinline__ void rebuild_row3(T (&u)[18], T c3) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const int a = (j + 1) % 3, b = (j + 2) % 3;
+        // z = r1[a]*r2[b] - r1[b]*r2[a];  row3[j] = c3 * conj(z)
+        const T zr = u[2 * a] * u[6 + 2 * b] - u[2 * a + 1] * u[6 + 2 * b + 1]
+                   - u[2 * b] * u[6 + 2 * a] + u[2 * b + 1] * u[6 + 2 * a + 1];
+        const T zi = u[2 * a] * u[6 + 2 * b + 1] + u[2 * a + 1] * u[6 + 2 * b]
+                   - u[2 * b] * u[6 + 2 * a + 1] - u[2 * b + 1] * u[6 + 2 * a];
+        u[12 + 2 * j] = c3 * zr;
+        u[12 + 2 * j + 1] = -c3 * zi;
+    }
+}
+
+template <int RECON>
+__device__ __forceinline__ void load_link(const char *__restrict__ w, int Vh, int e,
+                                          double (&u)[18], double c3, uint64_t pol) {
+    const double2 *p = reinterpret_cast<const double2 *>(w) + e;
+#pragma unroll
+    for (int k = 0; k < RECON / 2; ++k) {
+        const double2 t = ld_stream(p + (size_t)k * Vh, pol);
+        u[2 * k] = t.x; u[2 * k + 1] = t.y;
+    }
+    if (RECON == 12) rebuild_row3(u, c3);
+}
+template <int RECON>
+__device__ __forceinline__ void load_link(const char *__restrict__ w, int Vh, int e,
+                                          float (&u)[18], float c3, uint64_t pol) {
+    const float4 *p = reinterpret_cast<const float4 *>(w) + e;
+#pragma unroll
+    for (int k = 0; k < RECON / 4; ++k) {
+        const float4 t = ld_stream(p + (size_t)k * Vh, pol);
+        u[4 * k] = t.x; u[4 * k + 1] = t.y; u[4 * k + 2] = t.z; u[4 * k + 3] = t.w;
+    }
+    if (RECON == 18) {
+        const float2 t = ld_stream(reinterpret_cast<const float2 *>(w + (size_t)Vh * 64) + e, pol);
+        u[16] = t.x; u[17] = t.y;
+    } else {
+        rebuild_row3(u, c3);
+    }
+}
+
+template <typename T>
+__device__ __forceinline__ void matvec_acc(const T (&u)[18], const T (&v)[6], T (&acc)[6]) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            const T ur = u[6 * i + 2 * j], ui = u[6 * i + 2 * j + 1];
+            acc[2 * i] += ur * v[2 * j] - ui * v[2 * j + 1];
+            acc[2 * i + 1] += ur * v[2 * j + 1] + ui * v[2 * j];
+        }
+}
+
+// bytes of one (parity, direction) link set
+template <typename T, int RECON>
+__device__ __host__ __forceinline__ size_t link_set_bytes(int Vh) {
+    return (size_t)Vh * RECON * sizeof(T);
+}
+
+// acc = (D in)(x) for the output site (e, par).  W: packed gauge base (both parities).
+template <typename T, int RECON>
+__device__ __forceinline__ void dslash_site(const Geom &g, const char *__restrict__ W,
+                                            const char *__restrict__ in, int par, int e,
+                                            T (&acc)[6]) {
+    const Site s = site_of(g, e, par);
+    const int Vh = g.Vh;
+    const uint64_t pol = policy_evict_first();
+    const char *wp = W + (size_t)par * 8 * link_set_bytes<T, RECON>(Vh);
+    const int x[4] = {s.x0, s.x1, s.x2, s.x3};
+    int stride = 1;
+    int phase_sum = 0;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) acc[i] = T(0);
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) {
+        const int Lmu = g.L[mu];
+        const int ef = (s.lex + stride - (x[mu] == Lmu - 1 ? Lmu * stride : 0)) >> 1;
+        const int eb = (s.lex - stride + (x[mu] == 0 ? Lmu * stride : 0)) >> 1;
+        T c3f = T(0), c3b = T(0);
+        if (RECON == 12) {
+            const T eta = (phase_sum & 1) ? T(-2) : T(2);
+            c3f = (mu == 3 && x[3] == Lmu - 1) ? -eta : eta;
+            c3b = (mu == 3 && x[3] == 0) ? eta : -eta;
+        }
+        T u[18], v[6];
+        load_link<RECON>(wp + (size_t)(2 * mu) * link_set_bytes<T, RECON>(Vh), Vh, e, u, c3f, pol);
+        load_vec(in, Vh, ef, v);
+        matvec_acc(u, v, acc);
+        load_link<RECON>(wp + (size_t)(2 * mu + 1) * link_set_bytes<T, RECON>(Vh), Vh, e, u, c3b, pol);
+        load_vec(in, Vh, eb, v);
+        matvec_acc(u, v, acc);
+        stride *= Lmu;
+        phase_sum += x[mu];
+    }
+}
+
+}  // namespace stag
