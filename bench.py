@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py — staggered Dslash + multi-shift CG on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c5|c3|c2] [--impl reference]
+
+One STEP = one pass of the whole hot path over one synthetic
+pseudo-fermion source: one multi-shift CG solve of (m^2 - D_eo D_oe + sigma_i) x_i = b with all its
+Dslash applications, reductions, scalar recurrences and shift updates.  Row a1 (gauge pack) is
+setup, done once and reported as `pack_ms`.  `value` = Dslash GFLOP/s sustained through the solve
+(570 flop/site x 2 Dslash/iteration x iterations x Vh / time): the BASELINE metric's first figure
+measured over the whole path; the CG time-to-solution and the standalone Dslash sweep are beside it.
+Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+WORKLOADS = {"c2": "c2_16x16x16x4", "c3": "c3_24x24x24x6", "c4": "c4_32x32x32x8", "c5": "c5_64x64x64x64"}
+FLOP_PER_SITE = 570                                   # BASELINE.json:north_star
+DSLASH_BYTES = {(0, 18): 1248, (0, 12): 864, (1, 18): 624, (1, 12): 432}
+NOMINAL_HBM_GBS = 8000.0                              # "8 TB/s roofline" of BASELINE.json:metric
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def cg_bytes_per_site(prec, recon, iters, iters_shift):
+    """Algorithmic bytes of one solve per even site: per iteration 2 Dslash +
+    p re-read (a3) + r,q,r (a5) + r (a6), plus x_i,p_i read+write for every iteration shift i was live."""
+    w = 8 if prec == 0 else 4
+    vec = 6 * w
+    per_iter = 2 * DSLASH_BYTES[(prec, recon)] + vec + 3 * vec + vec
+    return iters * per_iter + sum(iters_shift) * 4 * vec
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, "/tmp/stag_clocks_%d.csv" % os.getpid()
+
+    def start(self):
+        try:
+            self.f = open(self.path, "w")
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        self.f.close()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.path):
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower() == "active":
+                    reasons.add(n)
+        os.unlink(self.path)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def make_inputs(cfg):
+    import stag_inputs as si
+    t0 = time.time()
+    U = si.make_links(cfg)
+    srcs = [si.make_source(cfg, k) for k in range(cfg["nsrc"])]
+    return U, srcs, time.time() - t0
+
+
+# ---------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle, as it stands, on the host cores, on a BOUNDED sample
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(cfg, U, b, budget_s: float, threads: int = 1):
+    """Runs `m` oracle CG iterations of the same solve (maxiter = m; the oracle is otherwise untouched)
+    with m sized from one probe iteration so the sample costs about budget_s.  Returns (GFLOP/s in the
+    metric's accounting, seconds per iteration, m)."""
+    import oracle
+    oracle.set_threads(threads)
+    L, vh = cfg["L"], int(np.prod(cfg["L"])) // 2
+    t0 = time.time()
+    oracle.mshift_cg(L, U, b, cfg["mass"], cfg["shifts"], cfg["stops"][0], 1)
+    t1 = time.time() - t0
+    m = int(max(2, min(200, budget_s / max(t1, 1e-6))))
+    t0 = time.time()
+    res = oracle.mshift_cg(L, U, b, cfg["mass"], cfg["shifts"], cfg["stops"][0], m)
+    dt = time.time() - t0
+    iters = max(res["iters"], 1)
+    return 2 * FLOP_PER_SITE * vh * iters / dt / 1e9, dt / iters, iters
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import stag_inputs as si
+    cfg = si.get_config(WORKLOADS[args.workload])
+    U, srcs, _ = make_inputs(cfg)
+    steps, warm = args.steps, args.warmup
+    per_step = max(1.0, min(20.0, 150.0 / max(1, steps + warm)))
+    vals, spi, its = [], [], 0
+    for k in range(warm + steps):
+        g, s, its = oracle_sample(cfg, U, srcs[k % len(srcs)], per_step)
+        if k >= warm:
+            vals.append(g); spi.append(s)
+    value = float(np.mean(vals))
+    ms = float(np.mean(spi)) * its * 1e3
+    sample = "%d oracle multi-shift CG iterations (maxiter=%d) of the %s solve per step, 1 thread" % (
+        its, its, WORKLOADS[args.workload])
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": args.gpus,
+           "steps": steps, "warmup": warm, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": workload_config(cfg, args.workload, 0, 18),
+           "cpu_baseline": {"value": value, "unit": "GFLOP/s", "cores": 1, "kind": "oracle", "sample": sample},
+           "e2e": {"value": value, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "oracle_s_per_iteration": float(np.mean(spi))}
+    print(json.dumps(out))
+    return 0
+
+
+METRIC = "Dslash GFLOP/s (570 flop/site) sustained through the multi-shift CG solve; CG s/solve beside it"
+
+
+def workload_config(cfg, name, prec, recon):
+    L = cfg["L"]
+    return {"workload": "%s: %dx%dx%dx%d lattice, %s links, %d-shift multi-shift CG, m=%g, stop=%g, %d source(s)"
+            % (WORKLOADS[name], L[0], L[1], L[2], L[3], cfg["links"][0], len(cfg["shifts"]), cfg["mass"],
+               cfg["stops"][0], cfg["nsrc"]),
+            "prec": "f64" if prec == 0 else "f32", "recon": recon, "nshift": len(cfg["shifts"]),
+            "parallelism": "replicas (independent sources, replicated gauge; no collective)"}
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def time_dslash(torch, ctx, packed, prec, recon, a, b, launches=100, repeats=5, warm=10):
+    """SURVEY.md §8(d) protocol: warm-up launches, then CUDA events around `launches` back-to-back
+    launches ping-ponging D_oe / D_eo (outputs consumed), median of `repeats`.  Returns s per launch."""
+    def pair(n):
+        for _ in range(n // 2):
+            ctx.dslash_oe(packed, prec, recon, a, b)
+            ctx.dslash_eo(packed, prec, recon, b, a)
+    pair(warm)
+    ts = []
+    for _ in range(repeats):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        pair(launches)
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1) * 1e-3 / launches)
+    return statistics.median(ts)
+
+
+def dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, pack_ms, gen_s):
+    """--dslash-only: the SURVEY.md §8(d) Dslash bandwidth sweep alone (no CG), one JSON line."""
+    peak, peak_src = measured_peak_gbs()
+    del packed
+    canon = ctx.alloc(ctx.gauge_canonical_bytes())
+    ctx.gauge_load(U, canon)
+    torch.cuda.synchronize()
+    out = {"metric": "Dslash GFLOP/s & HBM GB/s", "workload": WORKLOADS[args.workload], "peak_gbs": peak,
+           "peak_source": peak_src, "pack_ms": pack_ms, "input_gen_s": gen_s, "dslash": {}}
+    for p_, r_ in ((stag.F64, 18), (stag.F64, 12), (stag.F32, 18), (stag.F32, 12)):
+        pk = ctx.alloc(ctx.gauge_packed_bytes(p_, r_))
+        ctx.gauge_pack(canon, pk, p_, r_)
+        a = ctx.upload_vector(srcs[0], p_)
+        b = ctx.alloc(ctx.vector_bytes(p_))
+        s_per = time_dslash(torch, ctx, pk, p_, r_, a, b, launches=args.dslash_launches)
+        gbs = DSLASH_BYTES[(p_, r_)] * vh / s_per / 1e9
+        out["dslash"]["%s-%d" % ("f64" if p_ == stag.F64 else "f32", r_)] = {
+            "us": s_per * 1e6, "gflops": FLOP_PER_SITE * vh / s_per / 1e9, "gbs_algorithmic": gbs,
+            "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak}
+        del pk, a, b
+    print(json.dumps(out))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import stag_inputs as si
+    import paper_1010_5433_b200 as stag
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    prec = stag.F64 if args.prec == "f64" else stag.F32
+    recon = args.recon
+    cfg = si.get_config(WORKLOADS[args.workload])
+    L = cfg["L"]
+    vh = int(np.prod(L)) // 2
+    shifts, nshift = cfg["shifts"], len(cfg["shifts"])
+    stop, maxiter = cfg["stops"][0], 100000
+
+    # ---- setup (a1): seeded synthetic inputs -> HBM, packed once --------------------------------
+    U, srcs, gen_s = make_inputs(cfg)
+    ctx = stag.Stag(L)
+    canon = ctx.alloc(ctx.gauge_canonical_bytes())
+    ctx.gauge_load(U, canon)
+    torch.cuda.synchronize()
+    packed = ctx.alloc(ctx.gauge_packed_bytes(prec, recon))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    ctx.gauge_pack(canon, packed, prec, recon)
+    e1.record()
+    torch.cuda.synchronize()
+    pack_ms = e0.elapsed_time(e1)
+    del canon
+    vb = ctx.vector_bytes(prec)
+    if args.dslash_only:
+        return dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, pack_ms, gen_s)
+    bdev = [ctx.upload_vector(s, prec) for s in srcs]
+    x = ctx.alloc(nshift * vb)
+    ws = ctx.alloc(ctx.cg_workspace_bytes(prec, nshift))
+
+    def solve(k):
+        rc, info = ctx.mshift_cg(packed, prec, recon, bdev[k % len(bdev)], cfg["mass"], shifts, stop, maxiter, x, ws)
+        if rc != 0:
+            raise RuntimeError("stag_mshift_cg rc=%d %r" % (rc, info))
+        return info
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- timed region: W warm-up solves, then exactly K solves ------------------------------------
+    for k in range(args.warmup):
+        solve(rank * args.steps + k)
+    clocks = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        clocks.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    infos = []
+    e0.record()
+    for k in range(args.steps):
+        infos.append(solve(rank * args.steps + k))
+    e1.record()
+    barrier()
+    clk = clocks.stop() if rank == 0 else None
+    t = torch.tensor([e0.elapsed_time(e1) * 1e-3], dtype=torch.float64, device="cuda")
+    work = torch.tensor([float(sum(i["iters"] for i in infos)),
+                         float(sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"]) for i in infos)),
+                         float(sum(i["kernel_launches"] for i in infos))], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(work, op=dist.ReduceOp.SUM)
+    secs = float(t.item())
+    tot_iters, tot_bytes_site, launches = (float(v) for v in work.tolist())
+    value = 2 * FLOP_PER_SITE * vh * tot_iters / secs / 1e9
+    nsolves = args.steps * world
+
+    # ---- e2e: the same step through the host-buffer call, H<->D copies inside the timed region ----
+    n6 = vh * 6
+    hb = [torch.from_numpy(s.view(np.float64).reshape(-1).copy()).pin_memory() for s in srcs]
+    hx = torch.empty(nshift * n6, dtype=torch.float64).pin_memory()
+    scratch = ctx.alloc(ctx.host_scratch_bytes(prec, nshift))
+    e2e_steps = max(1, min(args.steps, 3))
+    ctx.mshift_cg_host(packed, prec, recon, hb[0], cfg["mass"], shifts, stop, maxiter, hx, scratch)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    it_e2e = 0
+    for k in range(e2e_steps):
+        rc, info = ctx.mshift_cg_host(packed, prec, recon, hb[(rank * e2e_steps + k) % len(hb)], cfg["mass"],
+                                      shifts, stop, maxiter, hx, scratch)
+        it_e2e += info["iters"]
+    e1.record()
+    barrier()
+    te = torch.tensor([e0.elapsed_time(e1) * 1e-3], dtype=torch.float64, device="cuda")
+    ie = torch.tensor([float(it_e2e)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        dist.all_reduce(ie, op=dist.ReduceOp.SUM)
+    e2e_value = 2 * FLOP_PER_SITE * vh * float(ie.item()) / float(te.item()) / 1e9
+    del scratch, hx
+
+    # ---- roofline of the dominant kernel (the Dslash) and the sweep over storage variants ---------
+    peak, peak_src = measured_peak_gbs()
+    dslash = {}
+    roof = None
+    if rank == 0:
+        va, vb_ = ctx.alloc(ctx.vector_bytes(stag.F64)), ctx.alloc(ctx.vector_bytes(stag.F64))
+        for p_, r_ in ((stag.F64, 18), (stag.F64, 12), (stag.F32, 18), (stag.F32, 12)):
+            pk = packed if (p_, r_) == (prec, recon) else ctx.upload_gauge(U, p_, r_)
+            a = ctx.upload_vector(srcs[0], p_)
+            s_per = time_dslash(torch, ctx, pk, p_, r_, a, vb_ if p_ == stag.F64 else va)
+            gbs = DSLASH_BYTES[(p_, r_)] * vh / s_per / 1e9
+            dslash["%s-%d" % ("f64" if p_ == stag.F64 else "f32", r_)] = {
+                "us": s_per * 1e6, "gflops": FLOP_PER_SITE * vh / s_per / 1e9, "gbs_algorithmic": gbs,
+                "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak,
+                "bytes_per_site": DSLASH_BYTES[(p_, r_)]}
+            if (p_, r_) == (prec, recon):
+                roof = {"bound": "hbm", "kernel": "dslash_kernel<%s,%d> (stag_dslash_oe/eo, %d launches ping-pong)"
+                        % ("double" if p_ == stag.F64 else "float", r_, 100),
+                        "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
+                        "peak_source": peak_src, "frac_of_8tbs": gbs / NOMINAL_HBM_GBS,
+                        "algorithmic_bytes_per_launch": DSLASH_BYTES[(p_, r_)] * vh,
+                        "avg_launch_us": s_per * 1e6, "traffic": None}
+            if pk is not packed:
+                del pk
+        prof = os.path.join(ROOT, "profiles", "traffic_%s.json" % args.workload)
+        if os.path.exists(prof):                 # dram bytes per launch from the committed ncu capture
+            try:
+                roof["traffic"] = json.load(open(prof)).get("%s-%d" % (args.prec, recon))
+            except Exception:
+                pass
+
+    # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        g, s_it, m = oracle_sample(cfg, U, srcs[0], 12.0)
+        cpu = {"value": g, "unit": "GFLOP/s", "cores": 1, "kind": "oracle",
+               "sample": "%d oracle multi-shift CG iterations (maxiter=%d) of the same %d-shift solve, %.3f s/iteration"
+                         % (m, m, nshift, s_it)}
+
+    if rank == 0:
+        iters = [i["iters"] for i in infos]
+        cg_gbs = tot_bytes_site * vh / secs / 1e9
+        out = {"metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+               "warmup": args.warmup, "ms_per_step": secs * 1e3 / args.steps, "higher_is_better": True,
+               "scaling": "weak", "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
+               "config": dict(workload_config(cfg, args.workload, prec, recon),
+                              l2="working set (2 link sets + %d vectors = %.0f MB) larger than the 126 MB L2; no flush"
+                                 % (2 * nshift + 4, (ctx.gauge_packed_bytes(prec, recon) + (2 * nshift + 4) * vb) / 1e6)),
+               "cg": {"s_per_solve": secs / args.steps, "iters": iters, "us_per_iter": secs / (tot_iters / world) * 1e6,
+                      "gbs_algorithmic": cg_gbs, "pct_of_8tbs": 100 * cg_gbs / NOMINAL_HBM_GBS,
+                      "pct_of_measured": 100 * cg_gbs / peak, "solves": nsolves,
+                      "iters_shift_first_solve": infos[0]["iters_shift"]},
+               "dslash": dslash, "roofline": roof, "cpu_baseline": cpu,
+               "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
+                       "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": float(te.item()) / e2e_steps,
+                       "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},
+               "gpu_launches": int(launches), "clocks": clk, "pack_ms": pack_ms, "input_gen_s": gen_s}
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=8)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dslash-only", action="store_true", help="Dslash bandwidth sweep only (no CG)")
+    ap.add_argument("--dslash-launches", type=int, default=100)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                       # timing rule: W >= 3
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

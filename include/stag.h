@@ -86,6 +86,7 @@ typedef struct stag_cg_info {
     double rnorm2;                         /* iterated <r,r> of the base system at exit        */
     double resid_iter[STAG_MAX_SHIFTS];    /* iterated zeta_i*||r||/||b|| per shift at exit/freeze */
     int iters_shift[STAG_MAX_SHIFTS];      /* iteration at which shift i stopped being updated */
+    int kernel_launches;                   /* kernels this call put on the stream (incl. no-op tail) */
 } stag_cg_info;
 
 /* ---- context --------------------------------------------------------------------------- */

@@ -28,12 +28,14 @@ SYMBOLS = [
 class CgInfo(C.Structure):
     _fields_ = [("iters", C.c_int), ("converged", C.c_int), ("breakdown", C.c_int),
                 ("stagnated", C.c_int), ("bnorm2", C.c_double), ("rnorm2", C.c_double),
-                ("resid_iter", C.c_double * MAX_SHIFTS), ("iters_shift", C.c_int * MAX_SHIFTS)]
+                ("resid_iter", C.c_double * MAX_SHIFTS), ("iters_shift", C.c_int * MAX_SHIFTS),
+                ("kernel_launches", C.c_int)]
 
     def as_dict(self, nshift: int) -> dict:
         return dict(iters=self.iters, converged=bool(self.converged), breakdown=bool(self.breakdown),
                     stagnated=bool(self.stagnated), bnorm2=self.bnorm2, rnorm2=self.rnorm2,
-                    resid_iter=list(self.resid_iter[:nshift]), iters_shift=list(self.iters_shift[:nshift]))
+                    resid_iter=list(self.resid_iter[:nshift]), iters_shift=list(self.iters_shift[:nshift]),
+                    kernel_launches=self.kernel_launches)
 
 
 class StagError(RuntimeError):

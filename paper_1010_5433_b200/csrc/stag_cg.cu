@@ -273,8 +273,10 @@ static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, 
         cudaEventCreateWithFlags(&ev[1], cudaEventDisableTiming) != cudaSuccess)
         rc = STAG_ERR_CUDA;
     const int nbatch = (maxiter + batch - 1) / batch;
+    int launches = 1;
     for (int k = 0; k <= nbatch && rc == STAG_OK; ++k) {
         if (k < nbatch) {
+            launches += 4 * batch;
             if (gexec) {
                 if (cudaGraphLaunch(gexec, st) != cudaSuccess) rc = STAG_ERR_CUDA;
             } else {
@@ -297,6 +299,7 @@ static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, 
     if (rc) { cudaGetLastError(); return rc; }
 
     if (y) {
+        ++launches;
         cg_partial_fraction_kernel<T, Lz::BLOCK><<<L.grid, Lz::BLOCK, 0, st>>>(
             L.nchunk, static_cast<const char *>(b), L.x, L.x_stride, static_cast<char *>(y), L.state);
         STAG_CUDA_OK(cudaGetLastError());
@@ -311,6 +314,7 @@ static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, 
         info->stagnated = h->stagnated;
         info->bnorm2 = h->bb;
         info->rnorm2 = h->rr;
+        info->kernel_launches = launches;
         for (int i = 0; i < nshift; ++i) {
             info->resid_iter[i] = h->bb > 0.0 ? h->resid_shift[i] : 0.0;
             info->iters_shift[i] = h->iters_shift[i];

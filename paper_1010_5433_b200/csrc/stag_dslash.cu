@@ -11,8 +11,13 @@
 
 namespace stag {
 
+// Register budget: 64 per thread (1024 resident threads / SM, so that the 1024 CTAs of a
+// 32^3x8 lattice are one wave), except fp64 12-real whose row-3 rebuild needs ~100.
+template <typename T, int RECON, int BLOCK>
+constexpr int min_ctas() { return (sizeof(T) == 8 && RECON == 12 ? 512 : 1024) / BLOCK; }
+
 template <typename T, int RECON, int BLOCK, int MODE>
-__global__ void __launch_bounds__(BLOCK)
+__global__ void __launch_bounds__(BLOCK, (min_ctas<T, RECON, BLOCK>()))
 dslash_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ in,
               char *__restrict__ out, const int par, const char *__restrict__ p,
               CgState *__restrict__ state, double *__restrict__ partials) {

@@ -105,9 +105,24 @@ def links_unit(L) -> np.ndarray:
     return U
 
 
-def _chunks(n: int, step: int = 1 << 20):
+def _chunks(n: int, step: int = 1 << 16):
     for lo in range(0, n, step):
         yield lo, min(n, lo + step)
+
+
+def _for_chunks(n: int, fn) -> None:
+    """fn(lo, hi) over cache-sized chunks, on all host cores (numpy releases the GIL; the values
+    are a pure function of the index, so threading does not change them)."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    chunks = list(_chunks(n))
+    nt = min(len(chunks), os.cpu_count() or 1)
+    if nt <= 1:
+        for lo, hi in chunks:
+            fn(lo, hi)
+        return
+    with ThreadPoolExecutor(nt) as ex:
+        list(ex.map(lambda c: fn(*c), chunks))
 
 
 def links_haar(L, seed: int, out: np.ndarray | None = None) -> np.ndarray:
@@ -115,8 +130,10 @@ def links_haar(L, seed: int, out: np.ndarray | None = None) -> np.ndarray:
     n = 4 * volume(L)
     U = out if out is not None else np.empty((n, 3, 3), dtype=np.complex128)
     U = U.reshape(n, 3, 3)
-    for lo, hi in _chunks(n):
+    def fill(lo, hi):
         U[lo:hi] = su3_project(_gaussian_matrices(seed, 0, np.arange(lo, hi)))
+
+    _for_chunks(n, fill)
     return U.reshape(volume(L), 4, 3, 3)
 
 
@@ -140,12 +157,14 @@ def links_smooth(L, seed: int, eps: float) -> np.ndarray:
     n = 4 * volume(L)
     U = np.empty((n, 3, 3), dtype=np.complex128)
     eye = np.eye(3)
-    for lo, hi in _chunks(n):
+    def fill(lo, hi):
         G = _gaussian_matrices(seed, 0, np.arange(lo, hi)) * np.sqrt(0.5)
         H = 0.5 * (G + np.conj(np.swapaxes(G, -1, -2)))
         tr = np.trace(H, axis1=-2, axis2=-1).real / 3.0
         H = H - tr[:, None, None] * eye
         U[lo:hi] = su3_project(_expi(H, eps))
+
+    _for_chunks(n, fill)
     return U.reshape(volume(L), 4, 3, 3)
 
 
@@ -173,8 +192,14 @@ def apply_gauge_transform(L, U: np.ndarray, g: np.ndarray) -> np.ndarray:
 # ----------------------------------------------------------------------------
 def source_gaussian(L, seed: int, stream: int = 1) -> np.ndarray:
     """iid complex normal (re, im each N(0,1)) on one parity, [Vh][3]."""
-    z = normals(seed, stream, np.arange(half_volume(L)), 6).reshape(-1, 3, 2)
-    return np.ascontiguousarray(z[..., 0] + 1j * z[..., 1])
+    out = np.empty((half_volume(L), 3), dtype=np.complex128)
+
+    def fill(lo, hi):
+        z = normals(seed, stream, np.arange(lo, hi), 6).reshape(-1, 3, 2)
+        out[lo:hi] = z[..., 0] + 1j * z[..., 1]
+
+    _for_chunks(half_volume(L), fill)
+    return out
 
 
 def source_plane_wave(L, n, colour, parity: int = 0) -> np.ndarray:
