@@ -41,6 +41,21 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def committed_traffic(workload, variant):
+    """dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch, from the committed `ncu --set
+    full` capture (profiles/traffic.csv; text written by hand from the capture, never by this run)."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        with open(path, newline="") as f:
+            for row in csv.DictReader(f):
+                if row["workload"] == workload and row["variant"] == variant and "dslash" in row["kernel"]:
+                    return int(row["dram_bytes_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
 def cg_bytes_per_site(prec, recon, iters, iters_shift):
     """Algorithmic bytes of one solve per even site: per iteration 2 Dslash +
     p re-read (a3) + r,q,r (a5) + r (a6), plus x_i,p_i read+write for every iteration shift i was live."""
@@ -237,6 +252,9 @@ def run_ours(args):
     # ---- setup (a1): seeded synthetic inputs -> HBM, packed once --------------------------------
     U, srcs, gen_s = make_inputs(cfg)
     ctx = stag.Stag(L)
+    for kv in args.opt:                                   # tuning knobs of stag_set_option
+        k, v = kv.split("=")
+        ctx.set_option(k, int(v))
     canon = ctx.alloc(ctx.gauge_canonical_bytes())
     ctx.gauge_load(U, canon)
     torch.cuda.synchronize()
@@ -342,12 +360,7 @@ def run_ours(args):
                         "avg_launch_us": s_per * 1e6, "traffic": None}
             if pk is not packed:
                 del pk
-        prof = os.path.join(ROOT, "profiles", "traffic_%s.json" % args.workload)
-        if os.path.exists(prof):                 # dram bytes per launch from the committed ncu capture
-            try:
-                roof["traffic"] = json.load(open(prof)).get("%s-%d" % (args.prec, recon))
-            except Exception:
-                pass
+        roof["traffic"] = committed_traffic(args.workload, "%s-%d" % (args.prec, recon))
 
     # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
     cpu = None
@@ -374,7 +387,7 @@ def run_ours(args):
                "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
                        "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": float(te.item()) / e2e_steps,
                        "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},
-               "gpu_launches": int(launches), "clocks": clk, "pack_ms": pack_ms, "input_gen_s": gen_s}
+               "gpu_launches": int(launches), "options": args.opt, "clocks": clk, "pack_ms": pack_ms, "input_gen_s": gen_s}
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -393,6 +406,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--dslash-only", action="store_true", help="Dslash bandwidth sweep only (no CG)")
     ap.add_argument("--dslash-launches", type=int, default=100)
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT",
+                    help="stag_set_option knob, e.g. cg_persistent=0 (repeatable)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                       # timing rule: W >= 3

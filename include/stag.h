@@ -97,7 +97,9 @@ void stag_ctx_destroy(stag_ctx *ctx);
 const char *stag_strerror(int err);
 /* Tuning knobs (integers): "dslash_block" (threads per CTA: 64|128|256), "cg_check_every"
  * (iterations between convergence polls), "cg_graph" (0|1: replay iterations as a CUDA
- * graph), "cg_freeze" (0|1: stop updating converged shifts, reading A10). */
+ * graph), "cg_freeze" (0|1: stop updating converged shifts, reading A10),
+ * "cg_persistent" (1, default: lattices whose r, q, p_base slices fit in shared memory run the
+ * whole solve as one cooperative kernel; 0: always the multi-kernel path). */
 int stag_set_option(stag_ctx *ctx, const char *key, int value);
 int stag_get_option(const stag_ctx *ctx, const char *key, int *value);
 

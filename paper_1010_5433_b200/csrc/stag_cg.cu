@@ -201,48 +201,14 @@ struct CgLaunch {
     }
 };
 
-template <typename T>
-static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, const void *b,
-                  double mass, int nshift, const double *shifts, const double *residues,
-                  double residue0, double stop, int maxiter, void *x, void *y, void *workspace,
-                  stag_cg_info *info, cudaStream_t st) {
-    typedef CgLaunch<T> Lz;
-    Lz L;
-    L.ctx = ctx; L.packed = packed; L.prec = prec; L.recon = recon; L.st = st;
-    L.ws = static_cast<char *>(workspace);
-    cg_workspace_layout(ctx, prec, nshift, &L.lay);
-    L.state = reinterpret_cast<CgState *>(L.ws + L.lay.state);
-    L.partials = reinterpret_cast<double *>(L.ws + L.lay.partials);
-    L.x = static_cast<char *>(x);
-    L.x_stride = (size_t)ctx->g.Vh * vec_bytes_per_site(prec);
-    L.nshift = nshift;
-    L.nchunk = (long)ctx->g.Vh * 6 / Vec16<T>::n;
-    {
-        const long want = (L.nchunk + Lz::BLOCK - 1) / Lz::BLOCK;
-        const long cap = (long)ctx->num_sms * ctx->opt.cg_ctas_per_sm;
-        L.grid = (int)(want < cap ? want : cap);
-    }
-    int base = 0;
-    for (int i = 1; i < nshift; ++i)
-        if (shifts[i] < shifts[base]) base = i;
-    L.base = base;
 
-    // initial state, staged through the ctx's pinned buffer
-    CgState *h = static_cast<CgState *>(ctx->pinned_info);
-    memset(h, 0, sizeof(*h));
-    h->alpha_old = 1.0; h->beta_old = 0.0;
-    h->c0 = mass * mass + shifts[base];
-    h->stop = stop; h->residue0 = residue0;
-    for (int i = 0; i < nshift; ++i) {
-        h->delta[i] = shifts[i] - shifts[base];
-        h->zeta[i] = 1.0; h->theta[i] = 1.0; h->active[i] = 1;
-        h->residues[i] = residues ? residues[i] : 0.0;
-        h->resid_shift[i] = 1.0;
-    }
-    h->nshift = nshift; h->base = base; h->maxiter = maxiter;
-    h->freeze = ctx->opt.cg_freeze; h->fp32 = (prec == STAG_F32);
-    if (maxiter == 0) h->done = 2;
-    STAG_CUDA_OK(cudaMemcpyAsync(L.state, h, sizeof(CgState), cudaMemcpyHostToDevice, st));
+// multi-kernel path: four launches per iteration, batches replayed as a CUDA graph, the host
+// polls the device-latched `done` word once per batch.
+template <typename T>
+static int run_multikernel(const CgLaunch<T> &L, const void *b, void *y, int maxiter, int *launches_out) {
+    typedef CgLaunch<T> Lz;
+    const stag_ctx *ctx = L.ctx;
+    cudaStream_t st = L.st;
     cg_init_kernel<T, Lz::BLOCK><<<L.grid, Lz::BLOCK, 0, st>>>(
         L.nchunk, static_cast<const char *>(b), L.ws + L.lay.r, L.ws + L.lay.p, L.lay.vec_stride, L.x,
         L.x_stride, L.state, L.partials);
@@ -303,6 +269,65 @@ static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, 
         cg_partial_fraction_kernel<T, Lz::BLOCK><<<L.grid, Lz::BLOCK, 0, st>>>(
             L.nchunk, static_cast<const char *>(b), L.x, L.x_stride, static_cast<char *>(y), L.state);
         STAG_CUDA_OK(cudaGetLastError());
+    }
+    *launches_out = launches;
+    return STAG_OK;
+}
+
+template <typename T>
+static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, const void *b,
+                  double mass, int nshift, const double *shifts, const double *residues,
+                  double residue0, double stop, int maxiter, void *x, void *y, void *workspace,
+                  stag_cg_info *info, cudaStream_t st) {
+    typedef CgLaunch<T> Lz;
+    Lz L;
+    L.ctx = ctx; L.packed = packed; L.prec = prec; L.recon = recon; L.st = st;
+    L.ws = static_cast<char *>(workspace);
+    cg_workspace_layout(ctx, prec, nshift, &L.lay);
+    L.state = reinterpret_cast<CgState *>(L.ws + L.lay.state);
+    L.partials = reinterpret_cast<double *>(L.ws + L.lay.partials);
+    L.x = static_cast<char *>(x);
+    L.x_stride = (size_t)ctx->g.Vh * vec_bytes_per_site(prec);
+    L.nshift = nshift;
+    L.nchunk = (long)ctx->g.Vh * 6 / Vec16<T>::n;
+    {
+        const long want = (L.nchunk + Lz::BLOCK - 1) / Lz::BLOCK;
+        const long cap = (long)ctx->num_sms * ctx->opt.cg_ctas_per_sm;
+        L.grid = (int)(want < cap ? want : cap);
+    }
+    int base = 0;
+    for (int i = 1; i < nshift; ++i)
+        if (shifts[i] < shifts[base]) base = i;
+    L.base = base;
+
+    // initial state, staged through the ctx's pinned buffer
+    CgState *h = static_cast<CgState *>(ctx->pinned_info);
+    memset(h, 0, sizeof(*h));
+    h->alpha_old = 1.0; h->beta_old = 0.0;
+    h->c0 = mass * mass + shifts[base];
+    h->stop = stop; h->residue0 = residue0;
+    for (int i = 0; i < nshift; ++i) {
+        h->delta[i] = shifts[i] - shifts[base];
+        h->zeta[i] = 1.0; h->theta[i] = 1.0; h->active[i] = 1;
+        h->residues[i] = residues ? residues[i] : 0.0;
+        h->resid_shift[i] = 1.0;
+    }
+    h->nshift = nshift; h->base = base; h->maxiter = maxiter;
+    h->freeze = ctx->opt.cg_freeze; h->fp32 = (prec == STAG_F32);
+    if (maxiter == 0) h->done = 2;
+    STAG_CUDA_OK(cudaMemcpyAsync(L.state, h, sizeof(CgState), cudaMemcpyHostToDevice, st));
+    int launches = 0;
+    bool persistent = ctx->opt.cg_persistent != 0 && cg_persistent_fits(ctx, prec);
+    if (persistent) {
+        // small lattice: the whole solve is one cooperative launch (stag_cg_persist.cu)
+        const int prc = cg_persistent_dispatch(ctx, packed, prec, recon, b, x, L.x_stride, y, L.ws, L.lay, st);
+        if (prc == STAG_ERR_UNSUPPORTED) persistent = false;       // cannot be co-resident: multi-kernel path
+        else if (prc) { cudaGetLastError(); return prc; }
+        else launches = 1;
+    }
+    if (!persistent) {
+        const int mrc = run_multikernel(L, b, y, maxiter, &launches);
+        if (mrc) return mrc;
     }
     STAG_CUDA_OK(cudaMemcpyAsync(h, L.state, sizeof(CgState), cudaMemcpyDeviceToHost, st));
     STAG_CUDA_OK(cudaStreamSynchronize(st));

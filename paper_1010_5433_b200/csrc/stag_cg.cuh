@@ -133,4 +133,10 @@ int dslash_eo_fused_dispatch(const stag_ctx *ctx, const void *packed, int prec, 
 int dslash_oe_cg_dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon,
                           const void *p_even, void *w_odd, CgState *state, void *stream);
 
+// implemented in stag_cg_persist.cu: the whole solve as one cooperative kernel (small lattices)
+bool cg_persistent_fits(const stag_ctx *ctx, int prec);
+int cg_persistent_dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon,
+                           const void *b, void *x, size_t x_stride, void *y, char *ws,
+                           const CgLayout &lay, cudaStream_t st);
+
 }  // namespace stag

@@ -59,6 +59,8 @@ struct Options {
     int cg_graph;            // replay the iteration batch as a CUDA graph
     int cg_freeze;           // stop updating converged shifts (reading A10)
     int cg_ctas_per_sm;      // persistent grid size of the CG streaming kernels, per SM
+    int cg_persistent_threads;  // threads per CTA of the persistent kernel: 1024 (64 regs) | 512 (128 regs)
+    int cg_persistent;       // 1: whole solve as one cooperative kernel when r,q,p fit in shared memory; 0: never
 };
 
 }  // namespace stag
@@ -120,6 +122,25 @@ __device__ __forceinline__ float2 ld_stream(const float2 *p, uint64_t pol) {
 __device__ __forceinline__ double2 ld_reuse(const double2 *p) { return __ldg(p); }
 __device__ __forceinline__ float4 ld_reuse(const float4 *p) { return __ldg(p); }
 __device__ __forceinline__ float2 ld_reuse(const float2 *p) { return __ldg(p); }
+
+// Coherent (weak, L1-allocating) loads for data that other CTAs rewrite inside the same kernel
+// between grid barriers.  asm volatile: never turned into ld.global.nc, never hoisted over a barrier.
+__device__ __forceinline__ double2 ld_coherent(const double2 *p) {
+    double2 r;
+    asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ float4 ld_coherent(const float4 *p) {
+    float4 r;
+    asm volatile("ld.global.v4.f32 {%0,%1,%2,%3}, [%4];"
+                 : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ float2 ld_coherent(const float2 *p) {
+    float2 r;
+    asm volatile("ld.global.v2.f32 {%0,%1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p) : "memory");
+    return r;
+}
 
 // ---- block-wide sum of one double (deterministic for a fixed block size) ----------------------
 template <int BLOCK>

@@ -29,17 +29,24 @@ template <> struct Prec<float> {
 };
 
 // ---- colour-vector load / store in the device format ----------------------------------------
-__device__ __forceinline__ void load_vec(const char *__restrict__ v, int Vh, int e, double (&x)[6]) {
+// NC = true: the vector is constant for the whole kernel (read-only path, __ldg).  NC = false: it
+// is rewritten inside the same (persistent) kernel between grid barriers, so the loads must stay
+// inside the memory model: plain coherent ld.global (still L1-allocating).
+template <bool NC = true>
+__device__ __forceinline__ void load_vec(const char *v, int Vh, int e, double (&x)[6]) {
     const double2 *p = reinterpret_cast<const double2 *>(v) + e;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double2 t = ld_reuse(p + (size_t)c * Vh);
+        const double2 t = NC ? ld_reuse(p + (size_t)c * Vh) : ld_coherent(p + (size_t)c * Vh);
         x[2 * c] = t.x; x[2 * c + 1] = t.y;
     }
 }
-__device__ __forceinline__ void load_vec(const char *__restrict__ v, int Vh, int e, float (&x)[6]) {
-    const float4 a = ld_reuse(reinterpret_cast<const float4 *>(v) + e);
-    const float2 b = ld_reuse(reinterpret_cast<const float2 *>(v + (size_t)Vh * 16) + e);
+template <bool NC = true>
+__device__ __forceinline__ void load_vec(const char *v, int Vh, int e, float (&x)[6]) {
+    const float4 *pa = reinterpret_cast<const float4 *>(v) + e;
+    const float2 *pb = reinterpret_cast<const float2 *>(v + (size_t)Vh * 16) + e;
+    const float4 a = NC ? ld_reuse(pa) : ld_coherent(pa);
+    const float2 b = NC ? ld_reuse(pb) : ld_coherent(pb);
     x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = b.x; x[5] = b.y;
 }
 __device__ __forceinline__ void store_vec(char *__restrict__ v, int Vh, int e, const double (&x)[6]) {
@@ -118,10 +125,9 @@ __device__ __host__ __forceinline__ size_t link_set_bytes(int Vh) {
 }
 
 // acc = (D in)(x) for the output site (e, par).  W: packed gauge base (both parities).
-template <typename T, int RECON>
+template <typename T, int RECON, bool NC = true>
 __device__ __forceinline__ void dslash_site(const Geom &g, const char *__restrict__ W,
-                                            const char *__restrict__ in, int par, int e,
-                                            T (&acc)[6]) {
+                                            const char *in, int par, int e, T (&acc)[6]) {
     const Site s = site_of(g, e, par);
     const int Vh = g.Vh;
     const uint64_t pol = policy_evict_first();
@@ -144,10 +150,10 @@ __device__ __forceinline__ void dslash_site(const Geom &g, const char *__restric
         }
         T u[18], v[6];
         load_link<RECON>(wp + (size_t)(2 * mu) * link_set_bytes<T, RECON>(Vh), Vh, e, u, c3f, pol);
-        load_vec(in, Vh, ef, v);
+        load_vec<NC>(in, Vh, ef, v);
         matvec_acc(u, v, acc);
         load_link<RECON>(wp + (size_t)(2 * mu + 1) * link_set_bytes<T, RECON>(Vh), Vh, e, u, c3b, pol);
-        load_vec(in, Vh, eb, v);
+        load_vec<NC>(in, Vh, eb, v);
         matvec_acc(u, v, acc);
         stride *= Lmu;
         phase_sum += x[mu];

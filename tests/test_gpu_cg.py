@@ -14,10 +14,22 @@ def rel(a, b):
     return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
 
 
-@pytest.fixture(scope="module")
-def stag():
+@pytest.fixture(scope="module", params=["persistent", "multikernel"])
+def stag(request):
+    """The binding, with Stag(L) pinned to one of the two CG paths: the single cooperative launch
+    (stag_cg_persist.cu) or four launches per iteration (stag_cg.cu).  Both must pass every test."""
+    import types
+
     import paper_1010_5433_b200 as m
-    return m
+
+    def make(L):
+        ctx = m.Stag(L)
+        ctx.set_option("cg_persistent", 1 if request.param == "persistent" else 0)
+        return ctx
+
+    ns = types.SimpleNamespace(**{k: getattr(m, k) for k in dir(m) if not k.startswith("__")})
+    ns.Stag, ns.cg_path = make, request.param
+    return ns
 
 
 def gpu_cg(stag, ctx, packed, prec, recon, b, mass, shifts, stop, maxiter, residues=None, residue0=0.0,
@@ -30,6 +42,10 @@ def gpu_cg(stag, ctx, packed, prec, recon, b, mass, shifts, stop, maxiter, resid
     y = ctx.alloc(vb) if want_y else None
     rc, info = ctx.mshift_cg(packed, prec, recon, bdev, mass, shifts, stop, maxiter, x, ws,
                              residues=residues, residue0=residue0, y_even=y)
+    if getattr(stag, "cg_path", None) == "persistent":
+        assert info["kernel_launches"] == 1
+    elif maxiter > 0:
+        assert info["kernel_launches"] > 1
     xs = np.stack([ctx.download_vector(x, prec, i * vb) for i in range(n)])
     return rc, info, xs, (ctx.download_vector(y, prec) if want_y else None)
 
