@@ -41,15 +41,15 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def committed_traffic(workload, variant):
-    """dram__bytes_read.sum + dram__bytes_write.sum per Dslash launch, from the committed `ncu --set
-    full` capture (profiles/traffic.csv; text written by hand from the capture, never by this run)."""
+def committed_traffic(workload, variant, kernel="dslash"):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed `ncu
+    --set full` capture (profiles/traffic.csv; text written from the capture, never by this run)."""
     import csv
     path = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(path, newline="") as f:
             for row in csv.DictReader(f):
-                if row["workload"] == workload and row["variant"] == variant and "dslash" in row["kernel"]:
+                if row["workload"] == workload and row["variant"] == variant and kernel in row["kernel"]:
                     return int(row["dram_bytes_per_launch"])
     except Exception:
         pass
@@ -339,7 +339,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel (the Dslash) and the sweep over storage variants ---------
     peak, peak_src = measured_peak_gbs()
     dslash = {}
-    roof = None
+    roof = roof_dslash = None
     if rank == 0:
         va, vb_ = ctx.alloc(ctx.vector_bytes(stag.F64)), ctx.alloc(ctx.vector_bytes(stag.F64))
         for p_, r_ in ((stag.F64, 18), (stag.F64, 12), (stag.F32, 18), (stag.F32, 12)):
@@ -361,6 +361,20 @@ def run_ours(args):
             if pk is not packed:
                 del pk
         roof["traffic"] = committed_traffic(args.workload, "%s-%d" % (args.prec, recon))
+        roof_dslash = roof
+        if launches == nsolves:
+            # the whole solve ran as ONE kernel per step (stag_cg_persist.cu): that kernel is the dominant
+            # one.  Algorithmic bytes per launch = SURVEY.md §8(d): (2736 + 192 N_live) per even site and
+            # iteration (fp64-18), summed over the iterations of the solve; duration = CUDA events around
+            # the K launches of the timed region / K.
+            cg_bytes_launch = tot_bytes_site * vh / nsolves
+            cg_gbs_ = tot_bytes_site * vh / secs / 1e9 / world        # per GPU: ranks run concurrently
+            roof = {"bound": "hbm", "kernel": "cg_persistent_kernel<%s,%d> (one launch = one multi-shift solve)"
+                    % ("double" if prec == stag.F64 else "float", recon),
+                    "achieved": cg_gbs_, "peak": peak, "unit": "GB/s", "frac": cg_gbs_ / peak,
+                    "peak_source": peak_src, "frac_of_8tbs": cg_gbs_ / NOMINAL_HBM_GBS,
+                    "algorithmic_bytes_per_launch": cg_bytes_launch, "avg_launch_us": secs / args.steps * 1e6,
+                    "traffic": committed_traffic(args.workload, "%s-%d" % (args.prec, recon), "cg_persistent")}
 
     # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
     cpu = None
@@ -383,7 +397,7 @@ def run_ours(args):
                       "gbs_algorithmic": cg_gbs, "pct_of_8tbs": 100 * cg_gbs / NOMINAL_HBM_GBS,
                       "pct_of_measured": 100 * cg_gbs / peak, "solves": nsolves,
                       "iters_shift_first_solve": infos[0]["iters_shift"]},
-               "dslash": dslash, "roofline": roof, "cpu_baseline": cpu,
+               "dslash": dslash, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
                "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
                        "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": float(te.item()) / e2e_steps,
                        "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},

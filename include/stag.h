@@ -61,6 +61,7 @@ extern "C" {
 #endif
 
 #define STAG_MAX_SHIFTS 32
+#define STAG_MAX_RHS 4        /* sources per block solve (stag_mshift_cg_block) */
 
 enum {
     STAG_OK = 0,
@@ -95,11 +96,13 @@ typedef struct stag_cg_info {
 int stag_ctx_create(const int L[4], stag_ctx **out);
 void stag_ctx_destroy(stag_ctx *ctx);
 const char *stag_strerror(int err);
-/* Tuning knobs (integers): "dslash_block" (threads per CTA: 64|128|256), "cg_check_every"
+/* Tuning knobs (integers): "dslash_block" (threads per CTA: 64|128|256), "dslash_regs"
+ * (register budget per thread: 0 auto | 64 | 128 | 255), "cg_check_every"
  * (iterations between convergence polls), "cg_graph" (0|1: replay iterations as a CUDA
  * graph), "cg_freeze" (0|1: stop updating converged shifts, reading A10),
  * "cg_persistent" (1, default: lattices whose r, q, p_base slices fit in shared memory run the
- * whole solve as one cooperative kernel; 0: always the multi-kernel path). */
+ * whole solve as one cooperative kernel; 0: always the multi-kernel path),
+ * "cg_persistent_threads" (0 auto | 512 | 1024 threads per CTA of that kernel). */
 int stag_set_option(stag_ctx *ctx, const char *key, int value);
 int stag_get_option(const stag_ctx *ctx, const char *key, int *value);
 
@@ -151,6 +154,32 @@ int stag_mshift_cg(const stag_ctx *ctx, const void *packed, int prec, int recon,
                    const double *host_residues, double residue0, double stop, int maxiter,
                    void *x_even, void *y_even, void *workspace, stag_cg_info *info,
                    void *stream);
+
+/* ---- N1: the hopping term on nrhs (1 .. STAG_MAX_RHS) independent vectors with
+ * ONE read of the links.  in / out: nrhs contiguous device-format vectors (stride
+ * stag_vector_bytes); out_parity 0 = D_eo (even output, odd input), 1 = D_oe.  One launch, no sync. */
+int stag_dslash_block(const stag_ctx *ctx, const void *packed, int prec, int recon, int out_parity,
+                      int nrhs, const void *in, void *out, void *stream);
+
+/* ---- N1: block solve of nrhs INDEPENDENT sources — the paper's multiple
+ * pseudo-fermions — with the same mass, shifts, residues and stop.  One persistent
+ * kernel; each link is read once per Dslash for all nrhs sources (links are 92 % of the stencil's
+ * bytes); every source keeps its own scalars, shift freezing and convergence latch, so each
+ * result is what stag_mshift_cg returns for that source alone.
+ *   nrhs       1 .. STAG_MAX_RHS
+ *   b_even     nrhs contiguous device-format vectors (stride stag_vector_bytes)
+ *   x_even     out, [nrhs][nshift] contiguous vectors: x of source s, shift i at byte offset
+ *              (s*nshift + i) * stag_vector_bytes
+ *   y_even     nullable, nrhs contiguous vectors
+ *   workspace  stag_cg_block_workspace_bytes(ctx, prec, nshift, nrhs) bytes, 256-byte aligned
+ *   info       host, nullable, nrhs structs (kernel_launches is counted in info[0])
+ * Returns STAG_OK only if every source converged; else the worst of NOTCONV / BREAKDOWN. */
+size_t stag_cg_block_workspace_bytes(const stag_ctx *ctx, int prec, int nshift, int nrhs);
+int stag_mshift_cg_block(const stag_ctx *ctx, const void *packed, int prec, int recon, int nrhs,
+                         const void *b_even, double mass, int nshift, const double *host_shifts,
+                         const double *host_residues, double residue0, double stop, int maxiter,
+                         void *x_even, void *y_even, void *workspace, stag_cg_info *info,
+                         void *stream);
 
 /* ---- the same calls on HOST buffers in canonical fp64 format (copies inside) --------------
  * dev_scratch: stag_host_scratch_bytes(ctx, prec, nshift) bytes of device memory

@@ -13,7 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libstag_b200.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC"]
+OBJ = os.path.join(HERE, "build")
 
 
 def sources() -> list[str]:
@@ -35,11 +36,23 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return SO
+    from concurrent.futures import ThreadPoolExecutor
     nvcc = os.environ.get("NVCC", "nvcc")
+    os.makedirs(OBJ, exist_ok=True)
+    extra = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(src: str) -> str:          # one translation unit per worker: seconds, not a minute
+        obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".%d.o" % os.getpid())
+        subprocess.check_call([nvcc] + NVCC_FLAGS + extra + ["-c", "-o", obj, src])
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
+        objs = list(pool.map(compile_one, sources()))
     tmp = SO + ".tmp.%d" % os.getpid()
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + sources()
-    subprocess.check_call(cmd)
+    subprocess.check_call([nvcc] + NVCC_FLAGS[:2] + ["-shared", "-o", tmp] + objs)
     os.replace(tmp, SO)
+    for o in objs:
+        os.unlink(o)
     return SO
 
 

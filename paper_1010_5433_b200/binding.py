@@ -13,6 +13,7 @@ SO = os.path.join(HERE, "libstag_b200.so")
 F64, F32 = 0, 1
 RECON18, RECON12 = 18, 12
 MAX_SHIFTS = 32
+MAX_RHS = 4
 OK, ERR_BADARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOT_SU3, ERR_NOTCONV, ERR_BREAKDOWN = 0, -1, -2, -3, -4, -5, -6
 
 # every symbol include/stag.h declares
@@ -22,6 +23,7 @@ SYMBOLS = [
     "stag_vector_bytes", "stag_cg_workspace_bytes", "stag_host_scratch_bytes",
     "stag_gauge_load", "stag_gauge_pack", "stag_vector_pack", "stag_vector_unpack",
     "stag_dslash_eo", "stag_dslash_oe", "stag_mshift_cg", "stag_dslash_host", "stag_mshift_cg_host",
+    "stag_dslash_block", "stag_cg_block_workspace_bytes", "stag_mshift_cg_block",
 ]
 
 
@@ -76,6 +78,11 @@ def lib() -> C.CDLL:
     l.stag_vector_unpack.argtypes = [_vp, _vp, C.c_int, _vp, _vp]
     l.stag_dslash_eo.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, _vp, _vp]
     l.stag_dslash_oe.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, _vp, _vp]
+    l.stag_dslash_block.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp]
+    l.stag_cg_block_workspace_bytes.argtypes = [_vp, C.c_int, C.c_int, C.c_int]
+    l.stag_cg_block_workspace_bytes.restype = _sz
+    l.stag_mshift_cg_block.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
+                                       C.c_double, C.c_double, C.c_int, _vp, _vp, _vp, C.POINTER(CgInfo), _vp]
     l.stag_mshift_cg.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
                                  C.c_double, C.c_double, C.c_int, _vp, _vp, _vp, C.POINTER(CgInfo), _vp]
     l.stag_dslash_host.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp]
@@ -208,6 +215,31 @@ class Stag:
             raise StagError(rc, "stag_mshift_cg")
         return rc, info.as_dict(n)
 
+    # ---- N1: nrhs independent sources through one link read
+    def cg_block_workspace_bytes(self, prec, nshift, nrhs):
+        return lib().stag_cg_block_workspace_bytes(self._h, prec, nshift, nrhs)
+
+    def dslash_block(self, packed, prec, recon, out_parity, nrhs, vin, vout, stream=None):
+        rc = lib().stag_dslash_block(self._h, _ptr(packed), prec, recon, int(out_parity), int(nrhs),
+                                     _ptr(vin), _ptr(vout), _stream(stream))
+        if rc:
+            raise StagError(rc, "stag_dslash_block")
+
+    def mshift_cg_block(self, packed, prec, recon, nrhs, b_even, mass, shifts, stop, maxiter, x_even, workspace,
+                        residues=None, residue0=0.0, y_even=None, stream=None, check=True):
+        """Returns (rc, [info dict per source])."""
+        sh = _darr(shifts)
+        rs = _darr(residues)
+        infos = (CgInfo * int(nrhs))()
+        n = sh[1].size
+        rc = lib().stag_mshift_cg_block(self._h, _ptr(packed), prec, recon, int(nrhs), _ptr(b_even), float(mass),
+                                        n, sh[0], rs[0] if rs else None, float(residue0), float(stop),
+                                        int(maxiter), _ptr(x_even), _ptr(y_even), _ptr(workspace), infos,
+                                        _stream(stream))
+        if check and rc not in (OK, ERR_NOTCONV, ERR_BREAKDOWN):
+            raise StagError(rc, "stag_mshift_cg_block")
+        return rc, [infos[s].as_dict(n) for s in range(int(nrhs))]
+
     # ---- host-buffer variants
     def dslash_host(self, packed, prec, recon, out_parity, host_in, host_out, dev_scratch, stream=None):
         rc = lib().stag_dslash_host(self._h, _ptr(packed), prec, recon, int(out_parity), _ptr(host_in),
@@ -243,6 +275,14 @@ class Stag:
         self.gauge_pack(canon, packed, prec, recon)
         torch.cuda.current_stream().synchronize()
         return packed
+
+    def upload_vectors(self, vs, prec: int) -> torch.Tensor:
+        """several host canonical vectors -> contiguous device-format vectors (stride vector_bytes)."""
+        vb = self.vector_bytes(prec)
+        dev = self.alloc(len(vs) * vb)
+        for k, v in enumerate(vs):
+            dev[k * vb:(k + 1) * vb].copy_(self.upload_vector(v, prec))
+        return dev
 
     def upload_vector(self, v: np.ndarray, prec: int) -> torch.Tensor:
         """host canonical vector complex128 [Vh][3] -> device-format vector."""

@@ -1,0 +1,570 @@
+// stag_cg_persist.cuh — the whole multi-shift CG solve of R independent sources as ONE persistent
+// cooperative kernel (PAPER.md:125-129 shifted CG; "multiple pseudo-fermions" = the R
+// independent right-hand sides).
+//
+// For the lattices of the paper's runs (4 x 16^3 ... 8 x 32^3, 4 x 48^3) one
+// CG iteration moves only a few hundred MB, so four kernel launches per iteration — each with a
+// fill/drain ramp and, twice, a serial "last CTA" reduction tail — cost as much as 15 % of the
+// iteration.  Here one CTA per SM owns a fixed, contiguous range of sites for the whole solve:
+//
+//   phase A  w = D_oe p_base                on the CTA's odd sites   -> global (neighbours read it)
+//            grid barrier
+//   phase B  q = (m^2+sigma_0) p - D_eo w   on the CTA's even sites  -> q stays in SHARED memory
+//            per-CTA partial of Re<p,q>     -> global;  grid barrier
+//   phase C  every CTA adds the partials in the same order (bit-identical alpha everywhere),
+//            runs the a4 recurrences in its own shared memory, then r -= alpha q with r and q
+//            both in shared memory (a5 moves no HBM bytes at all); partial of <r,r>; grid barrier
+//   phase D  every CTA: beta, beta_i, zeta_i, convergence latch, freezing (a4, a7); then a6:
+//            the base shift first (p_base is what the neighbours need), ARRIVE at the barrier,
+//            the other live shifts' x_i, p_i streamed once, then WAIT — the barrier latency hides
+//            behind the shift updates.
+//
+// r, q and the CTA's own slice of p_base live in shared memory for the whole solve when they fit
+// (3 x 48 B x sites/SM x R: 129 KB at 32^3 x 8, R = 1); what does not fit (priority r, q, p) stays
+// in the global workspace.  All scalars are fp64 and never leave the SM; the host sees one launch
+// and one read-back.
+//
+// R > 1 (N1): thread = (site, source), source fastest.  The R threads of a site issue the SAME
+// link load (one request, broadcast), so the links — 92 % of the stencil's bytes — are read once
+// for R sources; every source has its own scalars, shift list and convergence latch, and a source
+// that has converged simply stops issuing work while the others finish.
+#pragma once
+
+#include "stag_cg.cuh"
+#include "stag_dslash.cuh"
+
+namespace stag {
+
+// ---- grid barrier: monotone counter, arrive / wait split ---------------------------------------
+// Safe only because the kernel is launched cooperatively (all CTAs co-resident).
+__device__ __forceinline__ void grid_arrive(unsigned int *bar) {
+    __syncthreads();                       // every thread's writes of this phase are issued
+    if (threadIdx.x == 0) {
+        __threadfence();                   // ... and ordered before the arrival (cumulative)
+        atomicAdd(bar, 1u);
+    }
+}
+__device__ __forceinline__ void grid_wait(unsigned int *bar, unsigned int target) {
+    if (threadIdx.x == 0) {
+        unsigned int v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while ((int)(v - target) < 0);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// ---- a vector slice resident in shared memory: `n` thread-private slots ---------------------------
+template <typename T> struct SVec;
+template <> struct SVec<double> {
+    double2 *a; int n;
+    __device__ __forceinline__ void init(unsigned char *base, int n_) { a = reinterpret_cast<double2 *>(base); n = n_; }
+    __device__ __forceinline__ void load(int slot, double (&x)[6]) const {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { const double2 t = a[c * n + slot]; x[2 * c] = t.x; x[2 * c + 1] = t.y; }
+    }
+    __device__ __forceinline__ void store(int slot, const double (&x)[6]) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) a[c * n + slot] = make_double2(x[2 * c], x[2 * c + 1]);
+    }
+};
+template <> struct SVec<float> {
+    float4 *a; float2 *b;
+    __device__ __forceinline__ void init(unsigned char *base, int n_) {
+        a = reinterpret_cast<float4 *>(base); b = reinterpret_cast<float2 *>(base + (size_t)n_ * 16);
+    }
+    __device__ __forceinline__ void load(int slot, float (&x)[6]) const {
+        const float4 u = a[slot]; const float2 v = b[slot];
+        x[0] = u.x; x[1] = u.y; x[2] = u.z; x[3] = u.w; x[4] = v.x; x[5] = v.y;
+    }
+    __device__ __forceinline__ void store(int slot, const float (&x)[6]) {
+        a[slot] = make_float4(x[0], x[1], x[2], x[3]); b[slot] = make_float2(x[4], x[5]);
+    }
+};
+
+// A CTA-owned slice of one vector: in shared memory when it fits, else in the global workspace
+// (read and written only by the owning thread, so plain loads and stores are coherent).
+template <typename T>
+struct Slice {
+    SVec<T> s;
+    char *g;          // this thread's source's global vector (device format)
+    bool res;
+    __device__ __forceinline__ void load(int slot, int Vh, int e, T (&x)[6]) const {
+        if (res) s.load(slot, x); else load_vec<false>(g, Vh, e, x);
+    }
+    __device__ __forceinline__ void store(int slot, int Vh, int e, const T (&x)[6]) {
+        if (res) s.store(slot, x); else store_vec(g, Vh, e, x);
+    }
+};
+
+// ---- streaming (evict-first) own-site access to x_i, p_i -----------------------------------------
+__device__ __forceinline__ void load_vec_cs(const char *v, int Vh, int e, double (&x)[6]) {
+    const double2 *p = reinterpret_cast<const double2 *>(v) + e;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { const double2 t = __ldcs(p + (size_t)c * Vh); x[2 * c] = t.x; x[2 * c + 1] = t.y; }
+}
+__device__ __forceinline__ void load_vec_cs(const char *v, int Vh, int e, float (&x)[6]) {
+    const float4 a = __ldcs(reinterpret_cast<const float4 *>(v) + e);
+    const float2 b = __ldcs(reinterpret_cast<const float2 *>(v + (size_t)Vh * 16) + e);
+    x[0] = a.x; x[1] = a.y; x[2] = a.z; x[3] = a.w; x[4] = b.x; x[5] = b.y;
+}
+__device__ __forceinline__ void store_vec_cs(char *v, int Vh, int e, const double (&x)[6]) {
+    double2 *p = reinterpret_cast<double2 *>(v) + e;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) __stcs(p + (size_t)c * Vh, make_double2(x[2 * c], x[2 * c + 1]));
+}
+__device__ __forceinline__ void store_vec_cs(char *v, int Vh, int e, const float (&x)[6]) {
+    __stcs(reinterpret_cast<float4 *>(v) + e, make_float4(x[0], x[1], x[2], x[3]));
+    __stcs(reinterpret_cast<float2 *>(v + (size_t)Vh * 16) + e, make_float2(x[4], x[5]));
+}
+
+// ---- per-CTA copy of one source's scalar state (every CTA carries the same values) ------------------
+template <typename T>
+struct Scalars {
+    double delta[STAG_MAX_SHIFTS], zeta[STAG_MAX_SHIFTS], theta[STAG_MAX_SHIFTS], theta_new[STAG_MAX_SHIFTS];
+    double resid[STAG_MAX_SHIFTS];
+    T ca[STAG_MAX_SHIFTS], cz[STAG_MAX_SHIFTS], cb[STAG_MAX_SHIFTS];   // alpha_i, zeta_i(new), beta_i of live shifts
+    int live[STAG_MAX_SHIFTS];                                           // compacted list, base excluded
+    int active[STAG_MAX_SHIFTS], iters_shift[STAG_MAX_SHIFTS];
+    double bb, rr, alpha, alpha_old, beta_old, best_rr, pq;
+    T a_base, z_base, b_base;
+    int nlive, iter, done, converged, breakdown, stagnated, since_best;
+    // done: 0 running | 1 this iteration's x/p update is the last | 2 over
+};
+
+// sum of the G per-CTA partials, same order in every CTA => bit-identical result everywhere.
+// Valid in every lane of the calling warp.
+__device__ __forceinline__ double grid_total(const double *part, int G) {
+    double t = 0.0;
+    for (int i = threadIdx.x & 31; i < G; i += 32) t += __ldcg(part + i);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    return t;
+}
+
+// per-source CTA sums: thread t contributes to source t % R; result for source s -> slot[s * G]
+template <int NT, int R>
+__device__ __forceinline__ void cta_partials(double v, double *red /* (NT/32)*R doubles */, double *slot, int G) {
+#pragma unroll
+    for (int o = 16; o >= R; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane < R) red[warp * R + lane] = v;      // lane < R holds the sum over lanes = lane (mod R)
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int s = 0; s < R; ++s) {
+            double t = lane < NT / 32 ? red[lane * R + s] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+            if (lane == 0) __stcg(slot + (size_t)s * G, t);
+        }
+    }
+}
+
+struct PersistArgs {
+    const char *W;        // packed gauge
+    const char *b;        // R sources, stride b_stride
+    size_t b_stride;
+    char *w;              // R odd-site scratch vectors (global), stride vec_stride
+    char *r_g, *q_g;      // R global homes of r, q (used when not resident), stride vec_stride
+    size_t vec_stride;
+    char *p;              // search directions [source][shift] (global), stride p_stride
+    size_t p_stride;
+    char *x;              // solutions [source][shift], stride x_stride
+    size_t x_stride;
+    char *y;              // nullable; R vectors, stride x_stride
+    CgState *state;       // R states, stride state_stride bytes
+    size_t state_stride;
+    double *partials;     // 2 * R * gridDim.x doubles
+    int S;                // sites per CTA (multiple of 32)
+    int nrhs;             // sources actually present (<= R)
+    int res_r, res_q, res_p;   // which slices are resident in shared memory
+};
+
+template <typename T, int RECON, int NT, int R>
+__global__ void __launch_bounds__(NT, 1)
+cg_persistent_kernel(const Geom g, const PersistArgs a) {
+    extern __shared__ __align__(16) unsigned char dyn[];
+    __shared__ Scalars<T> sc[R];
+    __shared__ double red[(NT / 32) * R];
+    __shared__ int n_running;
+
+    constexpr int LS = NT / R;                       // sites per pass of the CTA
+    const int tid = threadIdx.x, G = gridDim.x, Vh = g.Vh, S = a.S;
+    const int rhs = tid % R, l0 = tid / R;
+    const int e0 = min(Vh, (int)blockIdx.x * S), ns = min(Vh, e0 + S) - e0;
+    unsigned int *bar = &a.state->ticket;
+    unsigned int epoch = 0;
+    double *part_pq = a.partials, *part_rr = a.partials + (size_t)R * G;
+
+    CgState *st = reinterpret_cast<CgState *>(reinterpret_cast<char *>(a.state) + (size_t)rhs * a.state_stride);
+    const int nshift = a.state->nshift, base = a.state->base, maxiter = a.state->maxiter;   // same for every source
+    const int freeze = a.state->freeze, fp32 = a.state->fp32;
+    const double stop = a.state->stop;
+    const T c0 = (T)a.state->c0;
+
+    const char *b_r = a.b + (size_t)rhs * a.b_stride;
+    char *w_r = a.w + (size_t)rhs * a.vec_stride;
+    char *p_r = a.p + (size_t)rhs * nshift * a.p_stride;
+    char *x_r = a.x + (size_t)rhs * nshift * a.x_stride;
+    char *p_base = p_r + (size_t)base * a.p_stride;
+    char *x_base = x_r + (size_t)base * a.x_stride;
+
+    Slice<T> r_s, q_s, p_s;
+    {
+        const size_t slice = (size_t)S * R * 6 * sizeof(T);
+        unsigned char *d = dyn;
+        r_s.res = a.res_r != 0; r_s.g = a.r_g + (size_t)rhs * a.vec_stride;
+        if (r_s.res) { r_s.s.init(d, S * R); d += slice; }
+        q_s.res = a.res_q != 0; q_s.g = a.q_g + (size_t)rhs * a.vec_stride;
+        if (q_s.res) { q_s.s.init(d, S * R); d += slice; }
+        p_s.res = a.res_p != 0; p_s.g = p_base;
+        if (p_s.res) { p_s.s.init(d, S * R); d += slice; }
+    }
+    const bool present = rhs < a.nrhs;
+
+    // ---- start: x_i = 0, r = p_i = b, bb = <b,b> ---------------------------------------------------
+    if (tid < 32 * R && (tid & 31) < STAG_MAX_SHIFTS) {
+        const int s = tid >> 5, i = tid & 31;
+        const CgState *ss = reinterpret_cast<const CgState *>(reinterpret_cast<const char *>(a.state) + (size_t)s * a.state_stride);
+        const bool on = i < nshift && s < a.nrhs;
+        sc[s].delta[i] = on ? ss->delta[i] : 0.0;
+        sc[s].zeta[i] = 1.0; sc[s].theta[i] = 1.0; sc[s].theta_new[i] = 1.0;
+        sc[s].resid[i] = 1.0;
+        sc[s].active[i] = on ? 1 : 0;
+        sc[s].iters_shift[i] = 0;
+    }
+    {
+        double acc = 0.0;
+        if (present)
+            for (int ls = l0; ls < ns; ls += LS) {
+                const int e = e0 + ls, slot = ls * R + rhs;
+                T v[6], z[6] = {T(0), T(0), T(0), T(0), T(0), T(0)};
+                load_vec<true>(b_r, Vh, e, v);
+#pragma unroll
+                for (int k = 0; k < 6; ++k) acc += (double)v[k] * (double)v[k];
+                r_s.store(slot, Vh, e, v);
+                if (p_s.res) p_s.s.store(slot, v);
+                for (int i = 0; i < nshift; ++i) {
+                    if (i == base) store_vec(p_base, Vh, e, v);
+                    else store_vec_cs(p_r + (size_t)i * a.p_stride, Vh, e, v);
+                    store_vec_cs(x_r + (size_t)i * a.x_stride, Vh, e, z);
+                }
+            }
+        cta_partials<NT, R>(acc, red, part_rr + blockIdx.x, G);
+    }
+    grid_arrive(bar);
+    grid_wait(bar, ++epoch * G);
+    if (tid < 32 * R) {
+        const int s = tid >> 5;
+        const double bb = grid_total(part_rr + (size_t)s * G, G);
+        if ((tid & 31) == 0) {
+            Scalars<T> &c = sc[s];
+            c.bb = bb; c.rr = bb; c.best_rr = bb; c.alpha = 0.0; c.alpha_old = 1.0; c.beta_old = 0.0;
+            c.pq = 0.0; c.iter = 0; c.done = 0; c.converged = 0; c.breakdown = 0; c.stagnated = 0;
+            c.since_best = 0; c.nlive = 0;
+            if (s >= a.nrhs) c.done = 2;
+            else if (!(bb > 0.0)) { c.converged = (bb == 0.0); c.breakdown = !(bb == 0.0); c.done = 2; }
+            else if (maxiter <= 0) c.done = 2;
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int n = 0;
+        for (int s = 0; s < R; ++s) n += sc[s].done == 0;
+        n_running = n;
+    }
+    __syncthreads();
+
+    // ---- iterations -----------------------------------------------------------------------------------
+    while (n_running > 0) {
+        const bool act = sc[rhs].done == 0;          // this thread's source is still iterating
+
+        // phase A (a2): w = D_oe p_base on this CTA's odd sites
+        if (act)
+            for (int ls = l0; ls < ns; ls += LS) {
+                T acc[6];
+                dslash_site<T, RECON, false>(g, a.W, p_base, 1, e0 + ls, acc);
+                store_vec(w_r, Vh, e0 + ls, acc);
+            }
+        grid_arrive(bar);
+        grid_wait(bar, ++epoch * G);
+
+        // phase B (a3): q = c0 p - D_eo w, partial Re<p,q>
+        {
+            double dot = 0.0;
+            if (act)
+                for (int ls = l0; ls < ns; ls += LS) {
+                    const int e = e0 + ls, slot = ls * R + rhs;
+                    T acc[6], pv[6];
+                    dslash_site<T, RECON, false>(g, a.W, w_r, 0, e, acc);
+                    p_s.load(slot, Vh, e, pv);
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) {
+                        acc[k] = c0 * pv[k] - acc[k];
+                        dot += (double)pv[k] * (double)acc[k];
+                    }
+                    q_s.store(slot, Vh, e, acc);
+                }
+            cta_partials<NT, R>(dot, red, part_pq + blockIdx.x, G);
+        }
+        grid_arrive(bar);
+        grid_wait(bar, ++epoch * G);
+
+        // phase C (a4 after <p,q>, then a5): alpha, theta_new_i;  r -= alpha q;  partial <r,r>
+        if (tid < 32 * R) {
+            const int s = tid >> 5, i = tid & 31;
+            Scalars<T> &c = sc[s];
+            if (c.done == 0) {
+                const double pq = grid_total(part_pq + (size_t)s * G, G);
+                const double alpha = c.rr / pq;
+                const bool bad = !(pq > 0.0) || !isfinite(alpha);
+                const double k = alpha * c.beta_old / c.alpha_old;
+                __syncwarp();
+                if (!bad && i < nshift) {
+                    if (c.active[i] == 2) c.active[i] = 0;            // frozen at the previous iteration
+                    c.theta_new[i] = 1.0 / ((1.0 + c.delta[i] * alpha) + k * (1.0 - c.theta[i]));
+                }
+                if (i == 0) {
+                    c.pq = pq;
+                    if (bad) { c.breakdown = 1; c.done = 2; } else c.alpha = alpha;   // breakdown: no update
+                }
+            }
+        }
+        __syncthreads();
+        const bool act2 = act && sc[rhs].done == 0;
+        {
+            double acc = 0.0;
+            if (act2) {
+                const T na = (T)(-sc[rhs].alpha);
+                for (int ls = l0; ls < ns; ls += LS) {
+                    const int e = e0 + ls, slot = ls * R + rhs;
+                    T rv[6], qv[6];
+                    r_s.load(slot, Vh, e, rv);
+                    q_s.load(slot, Vh, e, qv);
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) {
+                        rv[k] = fma(na, qv[k], rv[k]);
+                        acc += (double)rv[k] * (double)rv[k];
+                    }
+                    r_s.store(slot, Vh, e, rv);
+                }
+            }
+            cta_partials<NT, R>(acc, red, part_rr + blockIdx.x, G);
+        }
+        grid_arrive(bar);
+        grid_wait(bar, ++epoch * G);
+
+        // phase D (a4 after <r,r>, a7 latch, a6)
+        if (tid < 32 * R) {
+            const int s = tid >> 5, i = tid & 31;
+            Scalars<T> &c = sc[s];
+            if (c.done == 0) {
+                const double rr_new = grid_total(part_rr + (size_t)s * G, G);
+                const double alpha = c.alpha;
+                const double beta = rr_new / c.rr;
+                const double rel = sqrt(rr_new / c.bb);
+                const int iter = c.iter + 1;
+                bool live = false;
+                double th = 1.0, z = 1.0;
+                __syncwarp();
+                if (i < nshift) {
+                    th = c.theta_new[i];
+                    z = c.zeta[i] * th;
+                    c.zeta[i] = z;
+                    c.theta[i] = th;
+                    if (c.active[i] != 0) {
+                        live = true;
+                        if (c.active[i] == 1) {
+                            c.resid[i] = z * rel;
+                            c.iters_shift[i] = iter;
+                            if (freeze && i != base && z * rel <= 0.1 * stop) c.active[i] = 2;
+                        }
+                    }
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, live && i != base);
+                if (live && i != base) {
+                    const int j = __popc(m & ((1u << i) - 1u));
+                    c.live[j] = i;
+                    c.ca[j] = (T)(alpha * th);
+                    c.cz[j] = (T)z;
+                    c.cb[j] = (T)(beta * th * th);
+                }
+                if (i == base) { c.a_base = (T)(alpha * th); c.z_base = (T)z; c.b_base = (T)(beta * th * th); }
+                if (i == 0) {
+                    c.nlive = __popc(m);
+                    c.alpha_old = alpha;
+                    c.beta_old = beta;
+                    c.rr = rr_new;
+                    c.iter = iter;
+                    int done = 0;
+                    if (rel <= stop) { c.converged = 1; done = 1; }
+                    else if (iter >= maxiter) done = 1;
+                    else if (!(rr_new == rr_new)) { c.breakdown = 1; done = 1; }
+                    else if (fp32) {                                     // reading A9
+                        if (rr_new < c.best_rr) { c.best_rr = rr_new; c.since_best = 0; }
+                        else if (++c.since_best >= 50) { c.stagnated = 1; done = 1; }
+                    }
+                    c.done = done;
+                }
+            }
+        }
+        __syncthreads();
+        if (act2) {   // base shift first: its new p is what phase A of the next iteration gathers
+            const T ab = sc[rhs].a_base, zb = sc[rhs].z_base, bb_ = sc[rhs].b_base;
+            for (int ls = l0; ls < ns; ls += LS) {
+                const int e = e0 + ls, slot = ls * R + rhs;
+                T rv[6], pv[6], xv[6];
+                load_vec_cs(x_base, Vh, e, xv);
+                r_s.load(slot, Vh, e, rv);
+                p_s.load(slot, Vh, e, pv);
+#pragma unroll
+                for (int k = 0; k < 6; ++k) {
+                    xv[k] = fma(ab, pv[k], xv[k]);
+                    pv[k] = fma(zb, rv[k], bb_ * pv[k]);
+                }
+                store_vec_cs(x_base, Vh, e, xv);
+                if (p_s.res) p_s.s.store(slot, pv);
+                store_vec(p_base, Vh, e, pv);
+            }
+        }
+        grid_arrive(bar);
+        if (act2) {
+            const Scalars<T> &c = sc[rhs];
+            const int n = c.nlive;
+            for (int ls = l0; ls < ns; ls += LS) {
+                const int e = e0 + ls, slot = ls * R + rhs;
+                T rv[6];
+                r_s.load(slot, Vh, e, rv);
+#pragma unroll 2
+                for (int j = 0; j < n; ++j) {
+                    char *xp = x_r + (size_t)c.live[j] * a.x_stride;
+                    char *pp = p_r + (size_t)c.live[j] * a.p_stride;
+                    const T aj = c.ca[j], zj = c.cz[j], bj = c.cb[j];
+                    T pv[6], xv[6];
+                    load_vec_cs(pp, Vh, e, pv);
+                    load_vec_cs(xp, Vh, e, xv);
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) {
+                        xv[k] = fma(aj, pv[k], xv[k]);
+                        pv[k] = fma(zj, rv[k], bj * pv[k]);
+                    }
+                    store_vec_cs(xp, Vh, e, xv);
+                    store_vec_cs(pp, Vh, e, pv);
+                }
+            }
+        }
+        __syncthreads();                               // every thread has read sc[].done / coefficients
+        if (tid == 0) {
+            int n = 0;
+            for (int s = 0; s < R; ++s) {
+                if (sc[s].done == 1) sc[s].done = 2;   // its last x/p update has just run
+                n += sc[s].done == 0;
+            }
+            n_running = n;
+        }
+        grid_wait(bar, ++epoch * G);                   // ends with __syncthreads: n_running, done visible
+    }
+
+    // ---- a7: y = residue0 b + sum_i residues_i x_i (own sites only: no barrier needed) ---------------
+    if (a.y && present) {
+        char *y_r = a.y + (size_t)rhs * a.x_stride;
+        const T r0 = (T)st->residue0;
+        for (int ls = l0; ls < ns; ls += LS) {
+            const int e = e0 + ls;
+            T bv[6], acc[6];
+            load_vec<true>(b_r, Vh, e, bv);
+#pragma unroll
+            for (int k = 0; k < 6; ++k) acc[k] = r0 * bv[k];
+            for (int i = 0; i < nshift; ++i) {
+                const T ri = (T)st->residues[i];
+                T xv[6];
+                load_vec_cs(x_r + (size_t)i * a.x_stride, Vh, e, xv);
+#pragma unroll
+                for (int k = 0; k < 6; ++k) acc[k] = fma(ri, xv[k], acc[k]);
+            }
+            store_vec(y_r, Vh, e, acc);
+        }
+    }
+
+    // ---- read-back state (every CTA holds the same scalars; CTA 0 writes them) -------------------------
+    if (blockIdx.x == 0 && tid < 32 * R && (tid >> 5) < a.nrhs) {
+        const int s = tid >> 5, i = tid & 31;
+        CgState *o = reinterpret_cast<CgState *>(reinterpret_cast<char *>(a.state) + (size_t)s * a.state_stride);
+        const Scalars<T> &c = sc[s];
+        if (i < nshift) {
+            o->zeta[i] = c.zeta[i];
+            o->theta[i] = c.theta[i];
+            o->resid_shift[i] = c.resid[i];
+            o->iters_shift[i] = c.iters_shift[i];
+            o->active[i] = c.active[i];
+        }
+        if (i == 0) {
+            o->bb = c.bb; o->rr = c.rr; o->pq = c.pq; o->alpha = c.alpha;
+            o->iter = c.iter; o->converged = c.converged; o->breakdown = c.breakdown;
+            o->stagnated = c.stagnated; o->done = 2;
+        }
+    }
+}
+
+// ---- host side ---------------------------------------------------------------------------------------
+static constexpr size_t kMaxDynSmem = 200 * 1024;     // of 227 KB; the rest: static scalars + L1
+
+// sites per CTA for a grid of `grid` CTAs (multiple of 32: every CTA's slice starts on a 512-byte line)
+inline int sites_per_cta(int Vh, int grid) {
+    const int s = (Vh + grid - 1) / grid;
+    return (s + 31) & ~31;
+}
+
+template <typename T, int RECON, int NT, int R>
+int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t st) {
+    const Geom &g = ctx->g;
+    int grid = ctx->num_sms;
+    const int tiles = (g.Vh + 31) / 32;
+    if (grid > tiles) grid = tiles;
+    PersistArgs a = args;
+    a.S = sites_per_cta(g.Vh, grid);
+    // residency: as many of r, q, p (in that order of bytes saved) as fit
+    const size_t slice = (size_t)a.S * R * 6 * sizeof(T);
+    const int fit = (int)(kMaxDynSmem / slice);
+    a.res_r = fit >= 1; a.res_q = fit >= 2; a.res_p = fit >= 3;
+    const size_t smem = slice * (size_t)(a.res_r + a.res_q + a.res_p);
+    auto kern = cg_persistent_kernel<T, RECON, NT, R>;
+    STAG_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    STAG_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
+    if (per_sm < 1) return STAG_ERR_UNSUPPORTED;
+    Geom gg = g;
+    void *params[] = {(void *)&gg, (void *)&a};
+    STAG_CUDA_OK(cudaLaunchCooperativeKernel((const void *)kern, dim3(grid), dim3(NT), params, smem, st));
+    return STAG_OK;
+}
+
+// one explicit-instantiation translation unit per R (parallel compilation)
+template <int R>
+int cg_persistent_launch_r(const stag_ctx *ctx, int prec, int recon, const PersistArgs &a, cudaStream_t st);
+
+#define STAG_DEFINE_PERSIST_R(RR)                                                                       \
+    template <>                                                                                         \
+    int cg_persistent_launch_r<RR>(const stag_ctx *ctx, int prec, int recon, const PersistArgs &a,      \
+                                   cudaStream_t st) {                                                   \
+        /* 1024 threads x 64 registers or 512 x 128 per SM.  Measured at 32^3 x 8 (profiles/README.md): \
+           fp64 is faster with 512 x 128 (no spills, deeper per-thread load queue; fp64 12-real needs   \
+           ~100 registers anyway), fp32 with 1024 x 64.  cg_persistent_threads = 0 picks that. */       \
+        const int nt = ctx->opt.cg_persistent_threads;                                                  \
+        const bool wide = nt == 1024 || (nt == 0 && prec == STAG_F32);                                  \
+        if (prec == STAG_F64) {                                                                         \
+            if (recon == 12) return launch_persistent<double, 12, 512, RR>(ctx, a, st);                 \
+            return wide ? launch_persistent<double, 18, 1024, RR>(ctx, a, st)                           \
+                        : launch_persistent<double, 18, 512, RR>(ctx, a, st);                           \
+        }                                                                                               \
+        if (recon == 18)                                                                                \
+            return wide ? launch_persistent<float, 18, 1024, RR>(ctx, a, st)                            \
+                        : launch_persistent<float, 18, 512, RR>(ctx, a, st);                            \
+        return wide ? launch_persistent<float, 12, 1024, RR>(ctx, a, st)                                \
+                    : launch_persistent<float, 12, 512, RR>(ctx, a, st);                                \
+    }
+
+}  // namespace stag

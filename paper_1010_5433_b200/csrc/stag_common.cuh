@@ -54,12 +54,13 @@ __device__ __forceinline__ Site site_of(const Geom &g, int e, int par) {
 // ---- context -------------------------------------------------------------------------------
 struct Options {
     int dslash_block;        // threads per CTA of the Dslash kernels: 64 | 128 | 256
+    int dslash_regs;         // registers per thread: 64 (1024 resident threads / SM) | 128 (512) | 255 (256) | 0 auto
     int dslash_ctas_per_sm;  // 0: one CTA per block of sites; k > 0: persistent grid of k*SMs CTAs
     int cg_check_every;      // iterations between convergence polls (= iterations per CUDA graph)
     int cg_graph;            // replay the iteration batch as a CUDA graph
     int cg_freeze;           // stop updating converged shifts (reading A10)
     int cg_ctas_per_sm;      // persistent grid size of the CG streaming kernels, per SM
-    int cg_persistent_threads;  // threads per CTA of the persistent kernel: 1024 (64 regs) | 512 (128 regs)
+    int cg_persistent_threads;  // persistent-kernel CTA: 1024 threads (64 regs) | 512 (128 regs) | 0 auto
     int cg_persistent;       // 1: whole solve as one cooperative kernel when r,q,p fit in shared memory; 0: never
 };
 

@@ -26,13 +26,14 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
     g.dL1.init((uint32_t)L[1]);
     g.dL2.init((uint32_t)L[2]);
     c->opt.dslash_block = 128;
+    c->opt.dslash_regs = 0;
     c->opt.dslash_ctas_per_sm = 0;   // 0 = one CTA per 'dslash_block' sites (non-persistent)
     c->opt.cg_check_every = 16;
     c->opt.cg_graph = 1;
     c->opt.cg_freeze = 1;
     c->opt.cg_ctas_per_sm = 8;
     c->opt.cg_persistent = 1;
-    c->opt.cg_persistent_threads = 1024;
+    c->opt.cg_persistent_threads = 0;
     if (cudaGetDevice(&c->device) != cudaSuccess ||
         cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess ||
         cudaHostAlloc((void **)&c->pinned_flags, 64, cudaHostAllocMapped) != cudaSuccess ||
@@ -68,6 +69,7 @@ extern "C" const char *stag_strerror(int err) {
 static int *option_slot(Options &o, const char *key) {
     if (!key) return nullptr;
     if (!std::strcmp(key, "dslash_block")) return &o.dslash_block;
+    if (!std::strcmp(key, "dslash_regs")) return &o.dslash_regs;
     if (!std::strcmp(key, "dslash_ctas_per_sm")) return &o.dslash_ctas_per_sm;
     if (!std::strcmp(key, "cg_check_every")) return &o.cg_check_every;
     if (!std::strcmp(key, "cg_graph")) return &o.cg_graph;
@@ -84,8 +86,10 @@ extern "C" int stag_set_option(stag_ctx *ctx, const char *key, int value) {
     if (!slot) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.dslash_block && value != 64 && value != 128 && value != 256)
         return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.dslash_regs && value != 0 && value != 64 && value != 128 && value != 255)
+        return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_check_every && value < 1) return STAG_ERR_BADARG;
-    if (slot == &ctx->opt.cg_persistent_threads && value != 512 && value != 1024) return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.cg_persistent_threads && value != 0 && value != 512 && value != 1024) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_ctas_per_sm && (value < 1 || value > 16)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.dslash_ctas_per_sm && (value < 0 || value > 32)) return STAG_ERR_BADARG;
     *slot = value;

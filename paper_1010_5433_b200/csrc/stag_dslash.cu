@@ -13,11 +13,13 @@ namespace stag {
 
 // Register budget: 64 per thread (1024 resident threads / SM, so that the 1024 CTAs of a
 // 32^3x8 lattice are one wave), except fp64 12-real whose row-3 rebuild needs ~100.
-template <typename T, int RECON, int BLOCK>
-constexpr int min_ctas() { return (sizeof(T) == 8 && RECON == 12 ? 512 : 1024) / BLOCK; }
+// RT = resident threads per SM the kernel is compiled for: 1024 (64 registers each), 512 (128) or
+// 256 (255): fewer threads, each with a deeper queue of independent loads.
+template <int BLOCK, int RT>
+constexpr int min_ctas() { return RT / BLOCK > 0 ? RT / BLOCK : 1; }
 
-template <typename T, int RECON, int BLOCK, int MODE>
-__global__ void __launch_bounds__(BLOCK, (min_ctas<T, RECON, BLOCK>()))
+template <typename T, int RECON, int BLOCK, int MODE, int RT>
+__global__ void __launch_bounds__(BLOCK, (min_ctas<BLOCK, RT>()))
 dslash_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ in,
               char *__restrict__ out, const int par, const char *__restrict__ p,
               CgState *__restrict__ state, double *__restrict__ partials) {
@@ -54,6 +56,46 @@ dslash_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__
     }
 }
 
+// N1: R sources through one link read.  thread = (site, source), source fastest: the R threads of a
+// site issue the same link load (one request, broadcast by the LSU), each gathers its own source.
+template <typename T, int RECON, int BLOCK, int RT, int R>
+__global__ void __launch_bounds__(BLOCK, (min_ctas<BLOCK, RT>()))
+dslash_block_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ in,
+                    char *__restrict__ out, const int par, const size_t stride, const int nrhs) {
+    const long t = (long)blockIdx.x * BLOCK + threadIdx.x;
+    const int rhs = (int)(t % R), e = (int)(t / R);
+    if (e >= g.Vh || rhs >= nrhs) return;
+    T acc[6];
+    dslash_site<T, RECON>(g, W, in + (size_t)rhs * stride, par, e, acc);
+    store_vec(out + (size_t)rhs * stride, g.Vh, e, acc);
+}
+
+template <typename T, int RECON, int R>
+static int launch_dslash_block(const stag_ctx *ctx, const void *packed, const void *in, void *out, int par,
+                               int nrhs, cudaStream_t st) {
+    const Geom &g = ctx->g;
+    constexpr int BLOCK = 128;
+    const size_t stride = (size_t)g.Vh * 6 * sizeof(T);
+    const int grid = (int)(((long)g.Vh * R + BLOCK - 1) / BLOCK);
+    const char *W = static_cast<const char *>(packed);
+    if (sizeof(T) == 8)
+        dslash_block_kernel<T, RECON, BLOCK, 512, R><<<grid, BLOCK, 0, st>>>(
+            g, W, static_cast<const char *>(in), static_cast<char *>(out), par, stride, nrhs);
+    else
+        dslash_block_kernel<T, RECON, BLOCK, 1024, R><<<grid, BLOCK, 0, st>>>(
+            g, W, static_cast<const char *>(in), static_cast<char *>(out), par, stride, nrhs);
+    STAG_CUDA_OK(cudaGetLastError());
+    return STAG_OK;
+}
+
+template <typename T, int RECON>
+static int dslash_block_r(const stag_ctx *ctx, const void *packed, const void *in, void *out, int par,
+                          int nrhs, cudaStream_t st) {
+    if (nrhs == 1) return launch_dslash_block<T, RECON, 1>(ctx, packed, in, out, par, nrhs, st);
+    if (nrhs == 2) return launch_dslash_block<T, RECON, 2>(ctx, packed, in, out, par, nrhs, st);
+    return launch_dslash_block<T, RECON, 4>(ctx, packed, in, out, par, nrhs, st);
+}
+
 static int dslash_grid(const stag_ctx *ctx, int block, bool persistent_default) {
     const int tiles = (ctx->g.Vh + block - 1) / block;
     int per_sm = ctx->opt.dslash_ctas_per_sm;
@@ -74,17 +116,22 @@ static int launch_dslash(const stag_ctx *ctx, const void *packed, const void *in
     char *o = static_cast<char *>(out);
     const int block = ctx->opt.dslash_block;
     const int grid = dslash_grid(ctx, block, MODE == 2);
+    // dslash_regs = 0 (auto): measured best at 32^3x8 and 64^4 (profiles/README.md) — fp64 wants 128
+    // registers (18-real: no spills, deeper load queue; 12-real: the row-3 rebuild needs ~100),
+    // fp32 wants 64 and twice the threads.
+    int regs = ctx->opt.dslash_regs;
+    if (regs == 0) regs = sizeof(T) == 8 ? 128 : 64;
+    if (regs == 64 && sizeof(T) == 8 && RECON == 12) regs = 128;
+#define STAG_LAUNCH(B)                                                                                            \
+    if (regs == 64) dslash_kernel<T, RECON, B, MODE, 1024><<<grid, B, 0, st>>>(g, W, i, o, par, pp, state, partials);      \
+    else if (regs == 128) dslash_kernel<T, RECON, B, MODE, 512><<<grid, B, 0, st>>>(g, W, i, o, par, pp, state, partials); \
+    else dslash_kernel<T, RECON, B, MODE, 256><<<grid, B, 0, st>>>(g, W, i, o, par, pp, state, partials)
     switch (block) {
-        case 64:
-            dslash_kernel<T, RECON, 64, MODE><<<grid, 64, 0, st>>>(g, W, i, o, par, pp, state, partials);
-            break;
-        case 256:
-            dslash_kernel<T, RECON, 256, MODE><<<grid, 256, 0, st>>>(g, W, i, o, par, pp, state, partials);
-            break;
-        default:
-            dslash_kernel<T, RECON, 128, MODE><<<grid, 128, 0, st>>>(g, W, i, o, par, pp, state, partials);
-            break;
+        case 64: STAG_LAUNCH(64); break;
+        case 256: STAG_LAUNCH(256); break;
+        default: STAG_LAUNCH(128); break;
     }
+#undef STAG_LAUNCH
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
 }
@@ -122,6 +169,20 @@ int dslash_eo_fused_dispatch(const stag_ctx *ctx, const void *packed, int prec, 
 }
 
 }  // namespace stag
+
+extern "C" int stag_dslash_block(const stag_ctx *ctx, const void *packed, int prec, int recon,
+                                 int out_parity, int nrhs, const void *in, void *out, void *stream) {
+    using namespace stag;
+    if (!ctx || !packed || !in || !out || in == out) return STAG_ERR_BADARG;
+    if (!valid_prec(prec) || !valid_recon(recon) || (out_parity != 0 && out_parity != 1)) return STAG_ERR_BADARG;
+    if (nrhs < 1 || nrhs > STAG_MAX_RHS) return STAG_ERR_BADARG;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (prec == STAG_F64)
+        return recon == 18 ? dslash_block_r<double, 18>(ctx, packed, in, out, out_parity, nrhs, st)
+                           : dslash_block_r<double, 12>(ctx, packed, in, out, out_parity, nrhs, st);
+    return recon == 18 ? dslash_block_r<float, 18>(ctx, packed, in, out, out_parity, nrhs, st)
+                       : dslash_block_r<float, 12>(ctx, packed, in, out, out_parity, nrhs, st);
+}
 
 extern "C" int stag_dslash_eo(const stag_ctx *ctx, const void *packed, int prec, int recon,
                               const void *in_odd, void *out_even, void *stream) {
