@@ -149,7 +149,7 @@ def run_reference(args):
     cfg = si.get_config(WORKLOADS[args.workload])
     U, srcs, _ = make_inputs(cfg)
     steps, warm = args.steps, args.warmup
-    per_step = max(1.0, min(20.0, 150.0 / max(1, steps + warm)))
+    per_step = max(0.2, min(20.0, args.ref_seconds / max(1, steps + warm)))
     vals, spi, its = [], [], 0
     for k in range(warm + steps):
         g, s, its = oracle_sample(cfg, U, srcs[k % len(srcs)], per_step)
@@ -180,6 +180,26 @@ def workload_config(cfg, name, prec, recon):
                cfg["stops"][0], cfg["nsrc"]),
             "prec": "f64" if prec == 0 else "f32", "recon": recon, "nshift": len(cfg["shifts"]),
             "parallelism": "replicas (independent sources, replicated gauge; no collective)"}
+
+
+# ---------------------------------------------------------------------------------------------
+# N > 1: replicas only.  The two pieces of host logic the ranks share; covered on
+# CPU by tests/test_multirank_gloo.py (world_size 2, gloo).
+# ---------------------------------------------------------------------------------------------
+def source_for(rank: int, steps: int, k: int, nsrc: int) -> int:
+    """Which pseudo-fermion source rank `rank` solves at its step k: the sources are dealt
+    round-robin over the global step index, so ranks work on different sources."""
+    return (rank * steps + k) % nsrc
+
+
+def reduce_over_ranks(torch, dist, world: int, secs: float, work, device):
+    """Whole-job numbers: time = MAX over ranks, work = SUM over ranks.  No data-path collective."""
+    t = torch.tensor([secs], dtype=torch.float64, device=device)
+    w = torch.tensor([float(v) for v in work], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(w, op=dist.ReduceOp.SUM)
+    return float(t.item()), [float(v) for v in w.tolist()]
 
 
 # ---------------------------------------------------------------------------------------------
@@ -274,7 +294,7 @@ def run_ours(args):
     ws = ctx.alloc(ctx.cg_workspace_bytes(prec, nshift))
 
     def solve(k):
-        rc, info = ctx.mshift_cg(packed, prec, recon, bdev[k % len(bdev)], cfg["mass"], shifts, stop, maxiter, x, ws)
+        rc, info = ctx.mshift_cg(packed, prec, recon, bdev[k], cfg["mass"], shifts, stop, maxiter, x, ws)
         if rc != 0:
             raise RuntimeError("stag_mshift_cg rc=%d %r" % (rc, info))
         return info
@@ -286,7 +306,7 @@ def run_ours(args):
 
     # ---- timed region: W warm-up solves, then exactly K solves ------------------------------------
     for k in range(args.warmup):
-        solve(rank * args.steps + k)
+        solve(source_for(rank, args.steps, k, len(bdev)))
     clocks = ClockSampler(local)
     barrier()
     if rank == 0:
@@ -295,19 +315,15 @@ def run_ours(args):
     infos = []
     e0.record()
     for k in range(args.steps):
-        infos.append(solve(rank * args.steps + k))
+        infos.append(solve(source_for(rank, args.steps, k, len(bdev))))
     e1.record()
     barrier()
     clk = clocks.stop() if rank == 0 else None
-    t = torch.tensor([e0.elapsed_time(e1) * 1e-3], dtype=torch.float64, device="cuda")
-    work = torch.tensor([float(sum(i["iters"] for i in infos)),
-                         float(sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"]) for i in infos)),
-                         float(sum(i["kernel_launches"] for i in infos))], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(work, op=dist.ReduceOp.SUM)
-    secs = float(t.item())
-    tot_iters, tot_bytes_site, launches = (float(v) for v in work.tolist())
+    secs, (tot_iters, tot_bytes_site, launches) = reduce_over_ranks(
+        torch, dist, world, e0.elapsed_time(e1) * 1e-3,
+        [sum(i["iters"] for i in infos),
+         sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"]) for i in infos),
+         sum(i["kernel_launches"] for i in infos)], "cuda")
     value = 2 * FLOP_PER_SITE * vh * tot_iters / secs / 1e9
     nsolves = args.steps * world
 
@@ -323,17 +339,13 @@ def run_ours(args):
     e0.record()
     it_e2e = 0
     for k in range(e2e_steps):
-        rc, info = ctx.mshift_cg_host(packed, prec, recon, hb[(rank * e2e_steps + k) % len(hb)], cfg["mass"],
+        rc, info = ctx.mshift_cg_host(packed, prec, recon, hb[source_for(rank, e2e_steps, k, len(hb))], cfg["mass"],
                                       shifts, stop, maxiter, hx, scratch)
         it_e2e += info["iters"]
     e1.record()
     barrier()
-    te = torch.tensor([e0.elapsed_time(e1) * 1e-3], dtype=torch.float64, device="cuda")
-    ie = torch.tensor([float(it_e2e)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        dist.all_reduce(ie, op=dist.ReduceOp.SUM)
-    e2e_value = 2 * FLOP_PER_SITE * vh * float(ie.item()) / float(te.item()) / 1e9
+    te_s, (ie_sum,) = reduce_over_ranks(torch, dist, world, e0.elapsed_time(e1) * 1e-3, [it_e2e], "cuda")
+    e2e_value = 2 * FLOP_PER_SITE * vh * ie_sum / te_s / 1e9
     del scratch, hx
 
     # ---- roofline of the dominant kernel (the Dslash) and the sweep over storage variants ---------
@@ -399,7 +411,7 @@ def run_ours(args):
                       "iters_shift_first_solve": infos[0]["iters_shift"]},
                "dslash": dslash, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
                "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
-                       "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": float(te.item()) / e2e_steps,
+                       "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": te_s / e2e_steps,
                        "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},
                "gpu_launches": int(launches), "options": args.opt, "clocks": clk, "pack_ms": pack_ms, "input_gen_s": gen_s}
         print(json.dumps(out))
@@ -418,6 +430,8 @@ def main():
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-seconds", type=float, default=150.0,
+                    help="--impl reference: total oracle time budget over all steps")
     ap.add_argument("--dslash-only", action="store_true", help="Dslash bandwidth sweep only (no CG)")
     ap.add_argument("--dslash-launches", type=int, default=100)
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=INT",

@@ -24,10 +24,12 @@
 // in the global workspace.  All scalars are fp64 and never leave the SM; the host sees one launch
 // and one read-back.
 //
-// R > 1 (N1): thread = (site, source), source fastest.  The R threads of a site issue the SAME
-// link load (one request, broadcast), so the links — 92 % of the stencil's bytes — are read once
-// for R sources; every source has its own scalars, shift list and convergence latch, and a source
-// that has converged simply stops issuing work while the others finish.
+// R > 1 (N1): in the stencil phases (A, B) a thread owns one output site and ALL R sources: the 8
+// hopping matrices are loaded into registers once and applied to the R gathered neighbours, so the
+// links — 92 % of the stencil's bytes and most of its load instructions — are paid once for R
+// sources.  In the streaming phases (start, C, D, a7) the CTA's warps are split between the sources
+// (warp-uniform source, 32 consecutive sites per warp).  Every source has its own scalars, shift
+// list and convergence latch; a source that has converged stops issuing work while the others finish.
 #pragma once
 
 #include "stag_cg.cuh"
@@ -83,18 +85,20 @@ template <> struct SVec<float> {
     }
 };
 
-// A CTA-owned slice of one vector: in shared memory when it fits, else in the global workspace
-// (read and written only by the owning thread, so plain loads and stores are coherent).
+// A CTA-owned slice of one vector of each of the R sources: in shared memory when it fits (slot =
+// source * S + local site), else in the global workspace (read and written only by this CTA, with
+// a CTA barrier between phases, so plain loads and stores are coherent).
 template <typename T>
 struct Slice {
     SVec<T> s;
-    char *g;          // this thread's source's global vector (device format)
+    char *g;          // global home of source 0 (device format)
+    size_t gstride;   // bytes between the sources' global homes
     bool res;
-    __device__ __forceinline__ void load(int slot, int Vh, int e, T (&x)[6]) const {
-        if (res) s.load(slot, x); else load_vec<false>(g, Vh, e, x);
+    __device__ __forceinline__ void load(int slot, int r, int Vh, int e, T (&x)[6]) const {
+        if (res) s.load(slot, x); else load_vec<false>(g + (size_t)r * gstride, Vh, e, x);
     }
-    __device__ __forceinline__ void store(int slot, int Vh, int e, const T (&x)[6]) {
-        if (res) s.store(slot, x); else store_vec(g, Vh, e, x);
+    __device__ __forceinline__ void store(int slot, int r, int Vh, int e, const T (&x)[6]) {
+        if (res) s.store(slot, x); else store_vec(g + (size_t)r * gstride, Vh, e, x);
     }
 };
 
@@ -143,19 +147,48 @@ __device__ __forceinline__ double grid_total(const double *part, int G) {
     return t;
 }
 
-// per-source CTA sums: thread t contributes to source t % R; result for source s -> slot[s * G]
+// per-source CTA sums -> slot[s * G].  Two thread mappings:
+// "all": every thread holds one value per source (stencil phases)
 template <int NT, int R>
-__device__ __forceinline__ void cta_partials(double v, double *red /* (NT/32)*R doubles */, double *slot, int G) {
-#pragma unroll
-    for (int o = 16; o >= R; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+__device__ __forceinline__ void cta_partials_all(const double (&v)[R], double *red /* (NT/32)*R */, double *slot, int G) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double w[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        w[r] = v[r];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) w[r] += __shfl_xor_sync(0xffffffffu, w[r], o);
+    }
     __syncthreads();
-    if (lane < R) red[warp * R + lane] = v;      // lane < R holds the sum over lanes = lane (mod R)
+    if (lane == 0) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) red[warp * R + r] = w[r];
+    }
     __syncthreads();
     if (warp == 0) {
 #pragma unroll
         for (int s = 0; s < R; ++s) {
             double t = lane < NT / 32 ? red[lane * R + s] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+            if (lane == 0) __stcg(slot + (size_t)s * G, t);
+        }
+    }
+}
+// "stream": warp w works for source w / (NT/32/R) (streaming phases)
+template <int NT, int R>
+__device__ __forceinline__ void cta_partials_stream(double v, double *red /* NT/32 */, double *slot, int G) {
+    constexpr int WPS = NT / 32 / R;             // warps per source
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int s = 0; s < R; ++s) {
+            double t = lane < WPS ? red[s * WPS + lane] : 0.0;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
             if (lane == 0) __stcg(slot + (size_t)s * G, t);
@@ -191,9 +224,9 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
     __shared__ double red[(NT / 32) * R];
     __shared__ int n_running;
 
-    constexpr int LS = NT / R;                       // sites per pass of the CTA
+    constexpr int LS = NT / R;                       // streaming phases: sites per pass and source
     const int tid = threadIdx.x, G = gridDim.x, Vh = g.Vh, S = a.S;
-    const int rhs = tid % R, l0 = tid / R;
+    const int rhs = tid / LS, l0 = tid % LS;         // streaming phases: this thread's source (warp-uniform)
     const int e0 = min(Vh, (int)blockIdx.x * S), ns = min(Vh, e0 + S) - e0;
     unsigned int *bar = &a.state->ticket;
     unsigned int epoch = 0;
@@ -206,21 +239,22 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
     const T c0 = (T)a.state->c0;
 
     const char *b_r = a.b + (size_t)rhs * a.b_stride;
-    char *w_r = a.w + (size_t)rhs * a.vec_stride;
     char *p_r = a.p + (size_t)rhs * nshift * a.p_stride;
     char *x_r = a.x + (size_t)rhs * nshift * a.x_stride;
     char *p_base = p_r + (size_t)base * a.p_stride;
     char *x_base = x_r + (size_t)base * a.x_stride;
+    const size_t pb_stride = (size_t)nshift * a.p_stride;       // between the sources' p_base
+    char *p_base0 = a.p + (size_t)base * a.p_stride;            // p_base of source 0
 
     Slice<T> r_s, q_s, p_s;
     {
         const size_t slice = (size_t)S * R * 6 * sizeof(T);
         unsigned char *d = dyn;
-        r_s.res = a.res_r != 0; r_s.g = a.r_g + (size_t)rhs * a.vec_stride;
+        r_s.res = a.res_r != 0; r_s.g = a.r_g; r_s.gstride = a.vec_stride;
         if (r_s.res) { r_s.s.init(d, S * R); d += slice; }
-        q_s.res = a.res_q != 0; q_s.g = a.q_g + (size_t)rhs * a.vec_stride;
+        q_s.res = a.res_q != 0; q_s.g = a.q_g; q_s.gstride = a.vec_stride;
         if (q_s.res) { q_s.s.init(d, S * R); d += slice; }
-        p_s.res = a.res_p != 0; p_s.g = p_base;
+        p_s.res = a.res_p != 0; p_s.g = p_base0; p_s.gstride = pb_stride;
         if (p_s.res) { p_s.s.init(d, S * R); d += slice; }
     }
     const bool present = rhs < a.nrhs;
@@ -240,12 +274,12 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
         double acc = 0.0;
         if (present)
             for (int ls = l0; ls < ns; ls += LS) {
-                const int e = e0 + ls, slot = ls * R + rhs;
+                const int e = e0 + ls, slot = rhs * S + ls;
                 T v[6], z[6] = {T(0), T(0), T(0), T(0), T(0), T(0)};
                 load_vec<true>(b_r, Vh, e, v);
 #pragma unroll
                 for (int k = 0; k < 6; ++k) acc += (double)v[k] * (double)v[k];
-                r_s.store(slot, Vh, e, v);
+                r_s.store(slot, rhs, Vh, e, v);
                 if (p_s.res) p_s.s.store(slot, v);
                 for (int i = 0; i < nshift; ++i) {
                     if (i == base) store_vec(p_base, Vh, e, v);
@@ -253,7 +287,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                     store_vec_cs(x_r + (size_t)i * a.x_stride, Vh, e, z);
                 }
             }
-        cta_partials<NT, R>(acc, red, part_rr + blockIdx.x, G);
+        cta_partials_stream<NT, R>(acc, red, part_rr + blockIdx.x, G);
     }
     grid_arrive(bar);
     grid_wait(bar, ++epoch * G);
@@ -278,37 +312,58 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
     }
     __syncthreads();
 
+    // stencil phases: the R sources' input / output vectors
+    const char *pin[R];
+    const char *win[R];
+    char *wout[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        pin[r] = p_base0 + (size_t)r * pb_stride;
+        win[r] = a.w + (size_t)r * a.vec_stride;
+        wout[r] = a.w + (size_t)r * a.vec_stride;
+    }
+
     // ---- iterations -----------------------------------------------------------------------------------
     while (n_running > 0) {
-        const bool act = sc[rhs].done == 0;          // this thread's source is still iterating
+        const bool act = sc[rhs].done == 0;          // streaming phases: this thread's source is still iterating
+        unsigned mask = 0;                           // stencil phases: the sources still iterating
+#pragma unroll
+        for (int r = 0; r < R; ++r) mask |= (sc[r].done == 0 ? 1u : 0u) << r;
 
         // phase A (a2): w = D_oe p_base on this CTA's odd sites
-        if (act)
-            for (int ls = l0; ls < ns; ls += LS) {
-                T acc[6];
-                dslash_site<T, RECON, false>(g, a.W, p_base, 1, e0 + ls, acc);
-                store_vec(w_r, Vh, e0 + ls, acc);
-            }
+        for (int ls = tid; ls < ns; ls += NT) {
+            T acc[R][6];
+            dslash_site_multi<T, RECON, R, false>(g, a.W, pin, mask, 1, e0 + ls, acc);
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if (R == 1 || ((mask >> r) & 1u)) store_vec(wout[r], Vh, e0 + ls, acc[r]);
+        }
         grid_arrive(bar);
         grid_wait(bar, ++epoch * G);
 
         // phase B (a3): q = c0 p - D_eo w, partial Re<p,q>
         {
-            double dot = 0.0;
-            if (act)
-                for (int ls = l0; ls < ns; ls += LS) {
-                    const int e = e0 + ls, slot = ls * R + rhs;
-                    T acc[6], pv[6];
-                    dslash_site<T, RECON, false>(g, a.W, w_r, 0, e, acc);
-                    p_s.load(slot, Vh, e, pv);
+            double dot[R];
 #pragma unroll
-                    for (int k = 0; k < 6; ++k) {
-                        acc[k] = c0 * pv[k] - acc[k];
-                        dot += (double)pv[k] * (double)acc[k];
+            for (int r = 0; r < R; ++r) dot[r] = 0.0;
+            for (int ls = tid; ls < ns; ls += NT) {
+                const int e = e0 + ls;
+                T acc[R][6];
+                dslash_site_multi<T, RECON, R, false>(g, a.W, win, mask, 0, e, acc);
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+                    if (R == 1 || ((mask >> r) & 1u)) {
+                        T pv[6];
+                        p_s.load(r * S + ls, r, Vh, e, pv);
+#pragma unroll
+                        for (int k = 0; k < 6; ++k) {
+                            acc[r][k] = c0 * pv[k] - acc[r][k];
+                            dot[r] += (double)pv[k] * (double)acc[r][k];
+                        }
+                        q_s.store(r * S + ls, r, Vh, e, acc[r]);
                     }
-                    q_s.store(slot, Vh, e, acc);
-                }
-            cta_partials<NT, R>(dot, red, part_pq + blockIdx.x, G);
+            }
+            cta_partials_all<NT, R>(dot, red, part_pq + blockIdx.x, G);
         }
         grid_arrive(bar);
         grid_wait(bar, ++epoch * G);
@@ -340,19 +395,19 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             if (act2) {
                 const T na = (T)(-sc[rhs].alpha);
                 for (int ls = l0; ls < ns; ls += LS) {
-                    const int e = e0 + ls, slot = ls * R + rhs;
+                    const int e = e0 + ls, slot = rhs * S + ls;
                     T rv[6], qv[6];
-                    r_s.load(slot, Vh, e, rv);
-                    q_s.load(slot, Vh, e, qv);
+                    r_s.load(slot, rhs, Vh, e, rv);
+                    q_s.load(slot, rhs, Vh, e, qv);
 #pragma unroll
                     for (int k = 0; k < 6; ++k) {
                         rv[k] = fma(na, qv[k], rv[k]);
                         acc += (double)rv[k] * (double)rv[k];
                     }
-                    r_s.store(slot, Vh, e, rv);
+                    r_s.store(slot, rhs, Vh, e, rv);
                 }
             }
-            cta_partials<NT, R>(acc, red, part_rr + blockIdx.x, G);
+            cta_partials_stream<NT, R>(acc, red, part_rr + blockIdx.x, G);
         }
         grid_arrive(bar);
         grid_wait(bar, ++epoch * G);
@@ -415,11 +470,11 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
         if (act2) {   // base shift first: its new p is what phase A of the next iteration gathers
             const T ab = sc[rhs].a_base, zb = sc[rhs].z_base, bb_ = sc[rhs].b_base;
             for (int ls = l0; ls < ns; ls += LS) {
-                const int e = e0 + ls, slot = ls * R + rhs;
+                const int e = e0 + ls, slot = rhs * S + ls;
                 T rv[6], pv[6], xv[6];
                 load_vec_cs(x_base, Vh, e, xv);
-                r_s.load(slot, Vh, e, rv);
-                p_s.load(slot, Vh, e, pv);
+                r_s.load(slot, rhs, Vh, e, rv);
+                p_s.load(slot, rhs, Vh, e, pv);
 #pragma unroll
                 for (int k = 0; k < 6; ++k) {
                     xv[k] = fma(ab, pv[k], xv[k]);
@@ -435,9 +490,9 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             const Scalars<T> &c = sc[rhs];
             const int n = c.nlive;
             for (int ls = l0; ls < ns; ls += LS) {
-                const int e = e0 + ls, slot = ls * R + rhs;
+                const int e = e0 + ls, slot = rhs * S + ls;
                 T rv[6];
-                r_s.load(slot, Vh, e, rv);
+                r_s.load(slot, rhs, Vh, e, rv);
 #pragma unroll 2
                 for (int j = 0; j < n; ++j) {
                     char *xp = x_r + (size_t)c.live[j] * a.x_stride;
@@ -550,21 +605,25 @@ int cg_persistent_launch_r(const stag_ctx *ctx, int prec, int recon, const Persi
     template <>                                                                                         \
     int cg_persistent_launch_r<RR>(const stag_ctx *ctx, int prec, int recon, const PersistArgs &a,      \
                                    cudaStream_t st) {                                                   \
-        /* 1024 threads x 64 registers or 512 x 128 per SM.  Measured at 32^3 x 8 (profiles/README.md): \
-           fp64 is faster with 512 x 128 (no spills, deeper per-thread load queue; fp64 12-real needs   \
-           ~100 registers anyway), fp32 with 1024 x 64.  cg_persistent_threads = 0 picks that. */       \
-        const int nt = ctx->opt.cg_persistent_threads;                                                  \
-        const bool wide = nt == 1024 || (nt == 0 && prec == STAG_F32);                                  \
+        /* 1024 threads x 64 registers, 512 x 128 or (fp64) 256 x 255 per SM.  Measured at 32^3 x 8     \
+           (profiles/README.md): fp64 is fastest with 512 x 128 (deeper per-thread load queue; fp64     \
+           12-real needs ~100 registers anyway), fp32 with 1024 x 64, for R = 1 and R = 4 alike.        \
+           cg_persistent_threads = 0 picks that. */                                                     \
+        int nt = ctx->opt.cg_persistent_threads;                                                        \
+        if (nt == 0) nt = prec == STAG_F64 ? 512 : 1024;                                                \
         if (prec == STAG_F64) {                                                                         \
-            if (recon == 12) return launch_persistent<double, 12, 512, RR>(ctx, a, st);                 \
-            return wide ? launch_persistent<double, 18, 1024, RR>(ctx, a, st)                           \
-                        : launch_persistent<double, 18, 512, RR>(ctx, a, st);                           \
+            if (recon == 12)                                                                            \
+                return nt == 256 ? launch_persistent<double, 12, 256, RR>(ctx, a, st)                   \
+                                 : launch_persistent<double, 12, 512, RR>(ctx, a, st);                  \
+            return nt == 1024  ? launch_persistent<double, 18, 1024, RR>(ctx, a, st)                    \
+                   : nt == 256 ? launch_persistent<double, 18, 256, RR>(ctx, a, st)                     \
+                               : launch_persistent<double, 18, 512, RR>(ctx, a, st);                    \
         }                                                                                               \
         if (recon == 18)                                                                                \
-            return wide ? launch_persistent<float, 18, 1024, RR>(ctx, a, st)                            \
-                        : launch_persistent<float, 18, 512, RR>(ctx, a, st);                            \
-        return wide ? launch_persistent<float, 12, 1024, RR>(ctx, a, st)                                \
-                    : launch_persistent<float, 12, 512, RR>(ctx, a, st);                                \
+            return nt == 1024 ? launch_persistent<float, 18, 1024, RR>(ctx, a, st)                      \
+                              : launch_persistent<float, 18, 512, RR>(ctx, a, st);                      \
+        return nt == 1024 ? launch_persistent<float, 12, 1024, RR>(ctx, a, st)                          \
+                          : launch_persistent<float, 12, 512, RR>(ctx, a, st);                          \
     }
 
 }  // namespace stag

@@ -89,7 +89,7 @@ extern "C" int stag_set_option(stag_ctx *ctx, const char *key, int value) {
     if (slot == &ctx->opt.dslash_regs && value != 0 && value != 64 && value != 128 && value != 255)
         return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_check_every && value < 1) return STAG_ERR_BADARG;
-    if (slot == &ctx->opt.cg_persistent_threads && value != 0 && value != 512 && value != 1024) return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.cg_persistent_threads && value != 0 && value != 256 && value != 512 && value != 1024) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_ctas_per_sm && (value < 1 || value > 16)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.dslash_ctas_per_sm && (value < 0 || value > 32)) return STAG_ERR_BADARG;
     *slot = value;

@@ -56,18 +56,23 @@ dslash_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__
     }
 }
 
-// N1: R sources through one link read.  thread = (site, source), source fastest: the R threads of a
-// site issue the same link load (one request, broadcast by the LSU), each gathers its own source.
+// N1: R sources through one link read.  thread = one output site, ALL R sources: the 8 hopping
+// matrices are loaded into registers once and applied to the R gathered neighbours in turn, so both
+// the HBM bytes and the load-instruction count of the links are paid once per site, not per source.
 template <typename T, int RECON, int BLOCK, int RT, int R>
 __global__ void __launch_bounds__(BLOCK, (min_ctas<BLOCK, RT>()))
 dslash_block_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ in,
                     char *__restrict__ out, const int par, const size_t stride, const int nrhs) {
-    const long t = (long)blockIdx.x * BLOCK + threadIdx.x;
-    const int rhs = (int)(t % R), e = (int)(t / R);
-    if (e >= g.Vh || rhs >= nrhs) return;
-    T acc[6];
-    dslash_site<T, RECON>(g, W, in + (size_t)rhs * stride, par, e, acc);
-    store_vec(out + (size_t)rhs * stride, g.Vh, e, acc);
+    const int e = blockIdx.x * BLOCK + threadIdx.x;
+    if (e >= g.Vh) return;
+    const char *ins[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) ins[r] = in + (size_t)(r < nrhs ? r : 0) * stride;
+    T acc[R][6];
+    dslash_site_multi<T, RECON, R>(g, W, ins, (1u << nrhs) - 1u, par, e, acc);
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        if (r < nrhs) store_vec(out + (size_t)r * stride, g.Vh, e, acc[r]);
 }
 
 template <typename T, int RECON, int R>
@@ -76,14 +81,13 @@ static int launch_dslash_block(const stag_ctx *ctx, const void *packed, const vo
     const Geom &g = ctx->g;
     constexpr int BLOCK = 128;
     const size_t stride = (size_t)g.Vh * 6 * sizeof(T);
-    const int grid = (int)(((long)g.Vh * R + BLOCK - 1) / BLOCK);
+    const int grid = (g.Vh + BLOCK - 1) / BLOCK;
     const char *W = static_cast<const char *>(packed);
-    if (sizeof(T) == 8)
-        dslash_block_kernel<T, RECON, BLOCK, 512, R><<<grid, BLOCK, 0, st>>>(
-            g, W, static_cast<const char *>(in), static_cast<char *>(out), par, stride, nrhs);
-    else
-        dslash_block_kernel<T, RECON, BLOCK, 1024, R><<<grid, BLOCK, 0, st>>>(
-            g, W, static_cast<const char *>(in), static_cast<char *>(out), par, stride, nrhs);
+    // registers: R accumulators + one matrix + one neighbour.  fp64: 128 per thread up to R = 2, 255 at
+    // R = 4 (24 fp64 accumulators alone are 48 registers); fp32: 64 / 128.
+    constexpr int RT = sizeof(T) == 8 ? (R >= 4 ? 256 : 512) : (R >= 2 ? 512 : 1024);
+    dslash_block_kernel<T, RECON, BLOCK, RT, R><<<grid, BLOCK, 0, st>>>(
+        g, W, static_cast<const char *>(in), static_cast<char *>(out), par, stride, nrhs);
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
 }

@@ -124,10 +124,14 @@ __device__ __host__ __forceinline__ size_t link_set_bytes(int Vh) {
     return (size_t)Vh * RECON * sizeof(T);
 }
 
-// acc = (D in)(x) for the output site (e, par).  W: packed gauge base (both parities).
-template <typename T, int RECON, bool NC = true>
-__device__ __forceinline__ void dslash_site(const Geom &g, const char *__restrict__ W,
-                                            const char *in, int par, int e, T (&acc)[6]) {
+// acc[r] = (D in_r)(x) for the output site (e, par) and R independent source vectors in_r, with
+// ONE load of the 8 hopping matrices (N1: links are 92 % of the stencil's bytes;
+// the paper's multiple pseudo-fermions).  W: packed gauge base (both parities).
+// `mask` bit r = source r wanted (uniform over the CTA); the others cost nothing.
+template <typename T, int RECON, int R, bool NC = true>
+__device__ __forceinline__ void dslash_site_multi(const Geom &g, const char *__restrict__ W,
+                                                  const char *const (&in)[R], unsigned mask, int par,
+                                                  int e, T (&acc)[R][6]) {
     const Site s = site_of(g, e, par);
     const int Vh = g.Vh;
     const uint64_t pol = policy_evict_first();
@@ -136,7 +140,9 @@ __device__ __forceinline__ void dslash_site(const Geom &g, const char *__restric
     int stride = 1;
     int phase_sum = 0;
 #pragma unroll
-    for (int i = 0; i < 6; ++i) acc[i] = T(0);
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int i = 0; i < 6; ++i) acc[r][i] = T(0);
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) {
         const int Lmu = g.L[mu];
@@ -150,14 +156,33 @@ __device__ __forceinline__ void dslash_site(const Geom &g, const char *__restric
         }
         T u[18], v[6];
         load_link<RECON>(wp + (size_t)(2 * mu) * link_set_bytes<T, RECON>(Vh), Vh, e, u, c3f, pol);
-        load_vec<NC>(in, Vh, ef, v);
-        matvec_acc(u, v, acc);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (R == 1 || ((mask >> r) & 1u)) {
+                load_vec<NC>(in[r], Vh, ef, v);
+                matvec_acc(u, v, acc[r]);
+            }
         load_link<RECON>(wp + (size_t)(2 * mu + 1) * link_set_bytes<T, RECON>(Vh), Vh, e, u, c3b, pol);
-        load_vec<NC>(in, Vh, eb, v);
-        matvec_acc(u, v, acc);
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (R == 1 || ((mask >> r) & 1u)) {
+                load_vec<NC>(in[r], Vh, eb, v);
+                matvec_acc(u, v, acc[r]);
+            }
         stride *= Lmu;
         phase_sum += x[mu];
     }
+}
+
+// single source
+template <typename T, int RECON, bool NC = true>
+__device__ __forceinline__ void dslash_site(const Geom &g, const char *__restrict__ W,
+                                            const char *in, int par, int e, T (&acc)[6]) {
+    const char *const ins[1] = {in};
+    T a[1][6];
+    dslash_site_multi<T, RECON, 1, NC>(g, W, ins, 1u, par, e, a);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) acc[i] = a[0][i];
 }
 
 }  // namespace stag
