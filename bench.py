@@ -225,6 +225,61 @@ def time_dslash(torch, ctx, packed, prec, recon, a, b, launches=100, repeats=5, 
     return statistics.median(ts)
 
 
+def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
+    """N1: stag_dslash_block for R = 1, 2, 4 sources (100-launch ping-pong, as time_dslash) and ONE
+    stag_mshift_cg_block solve of min(4, nsrc) sources.  Algorithmic bytes per site of a block Dslash =
+    8 links (once) + R x (one read of the source + one write)."""
+    w = 8 if prec == stag.F64 else 4
+    vb = ctx.vector_bytes(prec)
+    out = {"dslash": {}, "cg": None}
+    for R in (1, 2, 4):
+        if R > len(srcs):
+            continue
+        a, b = ctx.upload_vectors(srcs[:R], prec), ctx.alloc(R * vb)
+
+        def pair(n):
+            for _ in range(n // 2):
+                ctx.dslash_block(packed, prec, recon, 1, R, a, b)
+                ctx.dslash_block(packed, prec, recon, 0, R, b, a)
+        pair(10)
+        ts = []
+        for _ in range(5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            pair(100)
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e-3 / 100)
+        s_per = statistics.median(ts)
+        bps = 8 * recon * w + 2 * 6 * w * R
+        gbs = bps * vh / s_per / 1e9
+        out["dslash"]["R%d" % R] = {"us": s_per * 1e6, "us_per_source": s_per * 1e6 / R,
+                                    "gflops": FLOP_PER_SITE * vh * R / s_per / 1e9, "bytes_per_site": bps,
+                                    "gbs_algorithmic": gbs, "pct_of_measured": 100 * gbs / peak}
+        del a, b
+    R = min(4, len(srcs))
+    n = len(cfg["shifts"])
+    stop = cfg["stops"][0] if prec == stag.F64 else max(cfg["stops"][0], 1e-5)
+    bdev = ctx.upload_vectors(srcs[:R], prec)
+    x = ctx.alloc(R * n * vb)
+    ws = ctx.alloc(ctx.cg_block_workspace_bytes(prec, n, R))
+    ts = []
+    for _ in range(2):                                    # first = warm-up
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        rc, infos = ctx.mshift_cg_block(packed, prec, recon, R, bdev, cfg["mass"], cfg["shifts"], stop, 100000, x, ws)
+        e1.record()
+        torch.cuda.synchronize()
+        ts.append(e0.elapsed_time(e1) * 1e-3)
+    its = [i["iters"] for i in infos]
+    out["cg"] = {"nrhs": R, "rc": rc, "s_per_block_solve": ts[-1], "s_per_source": ts[-1] / R, "iters": its,
+                 "us_per_iter": ts[-1] / max(its) * 1e6, "stop": stop,
+                 "gflops": 2 * FLOP_PER_SITE * vh * sum(its) / ts[-1] / 1e9,
+                 "call": "stag_mshift_cg_block (one persistent launch, links read once per Dslash for all sources)"}
+    return out
+
+
 def dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, pack_ms, gen_s):
     """--dslash-only: the SURVEY.md §8(d) Dslash bandwidth sweep alone (no CG), one JSON line."""
     peak, peak_src = measured_peak_gbs()
@@ -388,6 +443,11 @@ def run_ours(args):
                     "algorithmic_bytes_per_launch": cg_bytes_launch, "avg_launch_us": secs / args.steps * 1e6,
                     "traffic": committed_traffic(args.workload, "%s-%d" % (args.prec, recon), "cg_persistent")}
 
+    # ---- N1: the 4 pseudo-fermion sources of the workload through ONE link read ----
+    block = None
+    if rank == 0 and not args.no_block and len(srcs) >= 2:
+        block = measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak)
+
     # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -409,7 +469,7 @@ def run_ours(args):
                       "gbs_algorithmic": cg_gbs, "pct_of_8tbs": 100 * cg_gbs / NOMINAL_HBM_GBS,
                       "pct_of_measured": 100 * cg_gbs / peak, "solves": nsolves,
                       "iters_shift_first_solve": infos[0]["iters_shift"]},
-               "dslash": dslash, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
+               "dslash": dslash, "block": block, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
                "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
                        "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": te_s / e2e_steps,
                        "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},
@@ -430,6 +490,7 @@ def main():
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-block", action="store_true", help="skip the N1 multi-source measurements")
     ap.add_argument("--ref-seconds", type=float, default=150.0,
                     help="--impl reference: total oracle time budget over all steps")
     ap.add_argument("--dslash-only", action="store_true", help="Dslash bandwidth sweep only (no CG)")

@@ -97,8 +97,9 @@ int stag_ctx_create(const int L[4], stag_ctx **out);
 void stag_ctx_destroy(stag_ctx *ctx);
 const char *stag_strerror(int err);
 /* Tuning knobs (integers): "dslash_block" (threads per CTA: 64|128|256), "dslash_regs"
- * (register budget per thread: 0 auto | 64 | 128 | 255), "cg_check_every"
- * (iterations between convergence polls), "cg_graph" (0|1: replay iterations as a CUDA
+ * (register budget per thread: 0 auto | 64 | 128 | 255), "dslash_pipe" (1, default: stag_dslash_block
+ * streams the matrices through a cp.async shared-memory ring where that is faster; 0: never),
+ * "cg_check_every" (iterations between convergence polls), "cg_graph" (0|1: replay iterations as a CUDA
  * graph), "cg_freeze" (0|1: stop updating converged shifts, reading A10),
  * "cg_persistent" (1, default: lattices whose r, q, p_base slices fit in shared memory run the
  * whole solve as one cooperative kernel; 0: always the multi-kernel path),

@@ -56,6 +56,7 @@ struct Options {
     int dslash_block;        // threads per CTA of the Dslash kernels: 64 | 128 | 256
     int dslash_regs;         // registers per thread: 64 (1024 resident threads / SM) | 128 (512) | 255 (256) | 0 auto
     int dslash_ctas_per_sm;  // 0: one CTA per block of sites; k > 0: persistent grid of k*SMs CTAs
+    int dslash_pipe;         // stag_dslash_block: 1 = cp.async-ring kernel where it is the faster one (default); 0 = never
     int cg_check_every;      // iterations between convergence polls (= iterations per CUDA graph)
     int cg_graph;            // replay the iteration batch as a CUDA graph
     int cg_freeze;           // stop updating converged shifts (reading A10)

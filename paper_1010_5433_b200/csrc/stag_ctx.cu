@@ -28,6 +28,7 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
     c->opt.dslash_block = 128;
     c->opt.dslash_regs = 0;
     c->opt.dslash_ctas_per_sm = 0;   // 0 = one CTA per 'dslash_block' sites (non-persistent)
+    c->opt.dslash_pipe = 1;
     c->opt.cg_check_every = 16;
     c->opt.cg_graph = 1;
     c->opt.cg_freeze = 1;
@@ -71,6 +72,7 @@ static int *option_slot(Options &o, const char *key) {
     if (!std::strcmp(key, "dslash_block")) return &o.dslash_block;
     if (!std::strcmp(key, "dslash_regs")) return &o.dslash_regs;
     if (!std::strcmp(key, "dslash_ctas_per_sm")) return &o.dslash_ctas_per_sm;
+    if (!std::strcmp(key, "dslash_pipe")) return &o.dslash_pipe;
     if (!std::strcmp(key, "cg_check_every")) return &o.cg_check_every;
     if (!std::strcmp(key, "cg_graph")) return &o.cg_graph;
     if (!std::strcmp(key, "cg_freeze")) return &o.cg_freeze;

@@ -172,6 +172,10 @@ int dslash_eo_fused_dispatch(const stag_ctx *ctx, const void *packed, int prec, 
     return dispatch<2>(ctx, packed, prec, recon, w_odd, q_even, 0, p_even, state, partials, stream);
 }
 
+// implemented in stag_dslash_pipe.cu
+int dslash_pipe_dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon, int par, int nrhs,
+                         const void *in, void *out, cudaStream_t st);
+
 }  // namespace stag
 
 extern "C" int stag_dslash_block(const stag_ctx *ctx, const void *packed, int prec, int recon,
@@ -181,6 +185,10 @@ extern "C" int stag_dslash_block(const stag_ctx *ctx, const void *packed, int pr
     if (!valid_prec(prec) || !valid_recon(recon) || (out_parity != 0 && out_parity != 1)) return STAG_ERR_BADARG;
     if (nrhs < 1 || nrhs > STAG_MAX_RHS) return STAG_ERR_BADARG;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (ctx->opt.dslash_pipe != 0) {
+        const int rc = dslash_pipe_dispatch(ctx, packed, prec, recon, out_parity, nrhs, in, out, st);
+        if (rc != STAG_ERR_UNSUPPORTED) return rc;
+    }
     if (prec == STAG_F64)
         return recon == 18 ? dslash_block_r<double, 18>(ctx, packed, in, out, out_parity, nrhs, st)
                            : dslash_block_r<double, 12>(ctx, packed, in, out, out_parity, nrhs, st);

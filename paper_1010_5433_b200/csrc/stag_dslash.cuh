@@ -112,9 +112,12 @@ __device__ __forceinline__ void matvec_acc(const T (&u)[18], const T (&v)[6], T 
     for (int i = 0; i < 3; ++i)
 #pragma unroll
         for (int j = 0; j < 3; ++j) {
+            // four fused multiply-adds per complex multiply-accumulate (not mul + fma + add)
             const T ur = u[6 * i + 2 * j], ui = u[6 * i + 2 * j + 1];
-            acc[2 * i] += ur * v[2 * j] - ui * v[2 * j + 1];
-            acc[2 * i + 1] += ur * v[2 * j + 1] + ui * v[2 * j];
+            acc[2 * i] = fma(ur, v[2 * j], acc[2 * i]);
+            acc[2 * i] = fma(-ui, v[2 * j + 1], acc[2 * i]);
+            acc[2 * i + 1] = fma(ur, v[2 * j + 1], acc[2 * i + 1]);
+            acc[2 * i + 1] = fma(ui, v[2 * j], acc[2 * i + 1]);
         }
 }
 

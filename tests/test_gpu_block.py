@@ -24,9 +24,13 @@ def stag():
 @pytest.mark.parametrize("L", [(4, 4, 4, 4), (16, 16, 16, 4), (6, 4, 2, 8), (2, 2, 2, 2)])
 @pytest.mark.parametrize("prec,recon", [(0, 18), (0, 12), (1, 18), (1, 12)])
 @pytest.mark.parametrize("nrhs", [1, 2, 3, 4])
-def test_dslash_block_matches_oracle(stag, L, prec, recon, nrhs):
+@pytest.mark.parametrize("pipe", [1, 0])
+def test_dslash_block_matches_oracle(stag, L, prec, recon, nrhs, pipe):
+    """pipe = 1: the cp.async-ring kernel where the library picks it (fp64 R >= 3, fp32 R >= 2);
+    pipe = 0: the register-staged kernel everywhere."""
     U = si.links_haar(L, 21)
     ctx = stag.Stag(L)
+    ctx.set_option("dslash_pipe", pipe)
     packed = ctx.upload_gauge(U, prec, recon)
     vb = ctx.vector_bytes(prec)
     for par in (0, 1):

@@ -60,6 +60,45 @@ def test_c4_dslash_all_variants(stag, c4, prec, recon, regs):
     assert rel(ctx.download_vector(q, prec), oracle.dslash_eo(L, U, got_w)) <= TOL[prec]
 
 
+@pytest.mark.parametrize("prec,recon", [(0, 18), (0, 12), (1, 18), (1, 12)])
+@pytest.mark.parametrize("pipe", [1, 0])
+def test_c4_dslash_block_four_sources(stag, c4, prec, recon, pipe):
+    """N1 at full size, in the configuration bench.py times: the 4 pseudo-fermion sources of config 4
+    through one read of the links; every source compared element by element with the oracle."""
+    cfg, U, srcs = c4
+    L = cfg["L"]
+    ctx = stag.Stag(L)
+    ctx.set_option("dslash_pipe", pipe)
+    packed = ctx.upload_gauge(U, prec, recon)
+    vb = ctx.vector_bytes(prec)
+    vin, vout = ctx.upload_vectors(srcs, prec), ctx.alloc(4 * vb)
+    ctx.dslash_block(packed, prec, recon, 1, 4, vin, vout)
+    for k in range(4):
+        assert rel(ctx.download_vector(vout, prec, k * vb), oracle.dslash_oe(L, U, srcs[k])) <= TOL[prec]
+
+
+def test_c4_block_cg_four_sources(stag, c4):
+    """The block solve bench.py reports: 4 sources x 16 shifts in one persistent launch; true residual of
+    every (source, shift) by the oracle's operator, iteration counts equal to the single-source path's."""
+    cfg, U, srcs = c4
+    L, shifts, m, stop = cfg["L"], cfg["shifts"], cfg["mass"], cfg["stops"][0]
+    n = len(shifts)
+    ctx = stag.Stag(L)
+    packed = ctx.upload_gauge(U, 0, 18)
+    vb = ctx.vector_bytes(0)
+    x, ws = ctx.alloc(4 * n * vb), ctx.alloc(ctx.cg_block_workspace_bytes(0, n, 4))
+    rc, infos = ctx.mshift_cg_block(packed, 0, 18, 4, ctx.upload_vectors(srcs, 0), m, shifts, stop, 100000, x, ws)
+    assert rc == 0 and infos[0]["kernel_launches"] == 1
+    x1, ws1 = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(0, n))
+    for s, b in enumerate(srcs):
+        nb = np.linalg.norm(b)
+        for i in (0, 1, 5, 15):
+            xi = ctx.download_vector(x, 0, (s * n + i) * vb)
+            assert np.linalg.norm(b - oracle.apply_A(L, U, m, shifts[i], xi)) / nb <= stop, (s, i)
+        rc1, info1 = ctx.mshift_cg(packed, 0, 18, ctx.upload_vector(b, 0), m, shifts, stop, 100000, x1, ws1)
+        assert rc1 == 0 and abs(info1["iters"] - infos[s]["iters"]) <= 2
+
+
 @pytest.mark.parametrize("path", ["persistent", "multikernel"])
 def test_c4_multishift_cg_bench_configuration(stag, c4, path):
     """The solve bench.py times: 32^3x8, 16 shifts 1e-5..20, m = 0.01, stop 1e-10, fp64 18-real."""
