@@ -29,7 +29,10 @@ import numpy as np  # noqa: E402
 
 WORKLOADS = {"c2": "c2_16x16x16x4", "c3": "c3_24x24x24x6", "c4": "c4_32x32x32x8", "c5": "c5_64x64x64x64"}
 FLOP_PER_SITE = 570                                   # BASELINE.json:north_star
-DSLASH_BYTES = {(0, 18): 1248, (0, 12): 864, (1, 18): 624, (1, 12): 432}
+DSLASH_BYTES = {(0, 18): 1248, (0, 12): 864, (1, 18): 624, (1, 12): 432,
+                (2, 18): 1248, (2, 12): 864}                               # N3 split-double: 2 floats per real
+PREC_NAME = {0: "f64", 1: "f32", 2: "f64split"}
+VARIANTS = ((0, 18), (0, 12), (1, 18), (1, 12), (2, 18), (2, 12))
 NOMINAL_HBM_GBS = 8000.0                              # "8 TB/s roofline" of BASELINE.json:metric
 
 
@@ -59,7 +62,7 @@ def committed_traffic(workload, variant, kernel="dslash"):
 def cg_bytes_per_site(prec, recon, iters, iters_shift):
     """Algorithmic bytes of one solve per even site: per iteration 2 Dslash +
     p re-read (a3) + r,q,r (a5) + r (a6), plus x_i,p_i read+write for every iteration shift i was live."""
-    w = 8 if prec == 0 else 4
+    w = 4 if prec == 1 else 8
     vec = 6 * w
     per_iter = 2 * DSLASH_BYTES[(prec, recon)] + vec + 3 * vec + vec
     return iters * per_iter + sum(iters_shift) * 4 * vec
@@ -178,7 +181,7 @@ def workload_config(cfg, name, prec, recon):
     return {"workload": "%s: %dx%dx%dx%d lattice, %s links, %d-shift multi-shift CG, m=%g, stop=%g, %d source(s)"
             % (WORKLOADS[name], L[0], L[1], L[2], L[3], cfg["links"][0], len(cfg["shifts"]), cfg["mass"],
                cfg["stops"][0], cfg["nsrc"]),
-            "prec": "f64" if prec == 0 else "f32", "recon": recon, "nshift": len(cfg["shifts"]),
+            "prec": PREC_NAME[prec], "recon": recon, "nshift": len(cfg["shifts"]),
             "parallelism": "replicas (independent sources, replicated gauge; no collective)"}
 
 
@@ -229,7 +232,7 @@ def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
     """N1: stag_dslash_block for R = 1, 2, 4 sources (100-launch ping-pong, as time_dslash) and ONE
     stag_mshift_cg_block solve of min(4, nsrc) sources.  Algorithmic bytes per site of a block Dslash =
     8 links (once) + R x (one read of the source + one write)."""
-    w = 8 if prec == stag.F64 else 4
+    w = 4 if prec == stag.F32 else 8
     vb = ctx.vector_bytes(prec)
     out = {"dslash": {}, "cg": None}
     for R in (1, 2, 4):
@@ -260,7 +263,7 @@ def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
         del a, b
     R = min(4, len(srcs))
     n = len(cfg["shifts"])
-    stop = cfg["stops"][0] if prec == stag.F64 else max(cfg["stops"][0], 1e-5)
+    stop = cfg["stops"][0] if prec != stag.F32 else max(cfg["stops"][0], 1e-5)
     bdev = ctx.upload_vectors(srcs[:R], prec)
     x = ctx.alloc(R * n * vb)
     ws = ctx.alloc(ctx.cg_block_workspace_bytes(prec, n, R))
@@ -289,14 +292,14 @@ def dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, 
     torch.cuda.synchronize()
     out = {"metric": "Dslash GFLOP/s & HBM GB/s", "workload": WORKLOADS[args.workload], "peak_gbs": peak,
            "peak_source": peak_src, "pack_ms": pack_ms, "input_gen_s": gen_s, "dslash": {}}
-    for p_, r_ in ((stag.F64, 18), (stag.F64, 12), (stag.F32, 18), (stag.F32, 12)):
+    for p_, r_ in VARIANTS:
         pk = ctx.alloc(ctx.gauge_packed_bytes(p_, r_))
         ctx.gauge_pack(canon, pk, p_, r_)
         a = ctx.upload_vector(srcs[0], p_)
         b = ctx.alloc(ctx.vector_bytes(p_))
         s_per = time_dslash(torch, ctx, pk, p_, r_, a, b, launches=args.dslash_launches)
         gbs = DSLASH_BYTES[(p_, r_)] * vh / s_per / 1e9
-        out["dslash"]["%s-%d" % ("f64" if p_ == stag.F64 else "f32", r_)] = {
+        out["dslash"]["%s-%d" % (PREC_NAME[p_], r_)] = {
             "us": s_per * 1e6, "gflops": FLOP_PER_SITE * vh / s_per / 1e9, "gbs_algorithmic": gbs,
             "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak}
         del pk, a, b
@@ -316,7 +319,7 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    prec = stag.F64 if args.prec == "f64" else stag.F32
+    prec = {"f64": stag.F64, "f32": stag.F32, "f64split": stag.F64_SPLIT}[args.prec]
     recon = args.recon
     cfg = si.get_config(WORKLOADS[args.workload])
     L = cfg["L"]
@@ -409,18 +412,18 @@ def run_ours(args):
     roof = roof_dslash = None
     if rank == 0:
         va, vb_ = ctx.alloc(ctx.vector_bytes(stag.F64)), ctx.alloc(ctx.vector_bytes(stag.F64))
-        for p_, r_ in ((stag.F64, 18), (stag.F64, 12), (stag.F32, 18), (stag.F32, 12)):
+        for p_, r_ in VARIANTS:
             pk = packed if (p_, r_) == (prec, recon) else ctx.upload_gauge(U, p_, r_)
             a = ctx.upload_vector(srcs[0], p_)
-            s_per = time_dslash(torch, ctx, pk, p_, r_, a, vb_ if p_ == stag.F64 else va)
+            s_per = time_dslash(torch, ctx, pk, p_, r_, a, vb_ if p_ != stag.F32 else va)
             gbs = DSLASH_BYTES[(p_, r_)] * vh / s_per / 1e9
-            dslash["%s-%d" % ("f64" if p_ == stag.F64 else "f32", r_)] = {
+            dslash["%s-%d" % (PREC_NAME[p_], r_)] = {
                 "us": s_per * 1e6, "gflops": FLOP_PER_SITE * vh / s_per / 1e9, "gbs_algorithmic": gbs,
                 "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak,
                 "bytes_per_site": DSLASH_BYTES[(p_, r_)]}
             if (p_, r_) == (prec, recon):
                 roof = {"bound": "hbm", "kernel": "dslash_kernel<%s,%d> (stag_dslash_oe/eo, %d launches ping-pong)"
-                        % ("double" if p_ == stag.F64 else "float", r_, 100),
+                        % ("float" if p_ == stag.F32 else "double", r_, 100),
                         "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
                         "peak_source": peak_src, "frac_of_8tbs": gbs / NOMINAL_HBM_GBS,
                         "algorithmic_bytes_per_launch": DSLASH_BYTES[(p_, r_)] * vh,
@@ -437,7 +440,7 @@ def run_ours(args):
             cg_bytes_launch = tot_bytes_site * vh / nsolves
             cg_gbs_ = tot_bytes_site * vh / secs / 1e9 / world        # per GPU: ranks run concurrently
             roof = {"bound": "hbm", "kernel": "cg_persistent_kernel<%s,%d> (one launch = one multi-shift solve)"
-                    % ("double" if prec == stag.F64 else "float", recon),
+                    % ("float" if prec == stag.F32 else "double", recon),
                     "achieved": cg_gbs_, "peak": peak, "unit": "GB/s", "frac": cg_gbs_ / peak,
                     "peak_source": peak_src, "frac_of_8tbs": cg_gbs_ / NOMINAL_HBM_GBS,
                     "algorithmic_bytes_per_launch": cg_bytes_launch, "avg_launch_us": secs / args.steps * 1e6,
@@ -445,7 +448,7 @@ def run_ours(args):
 
     # ---- N1: the 4 pseudo-fermion sources of the workload through ONE link read ----
     block = None
-    if rank == 0 and not args.no_block and len(srcs) >= 2:
+    if rank == 0 and not args.no_block and len(srcs) >= 2 and prec != stag.F64_SPLIT:
         block = measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak)
 
     # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
@@ -461,7 +464,7 @@ def run_ours(args):
         cg_gbs = tot_bytes_site * vh / secs / 1e9
         out = {"metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": secs * 1e3 / args.steps, "higher_is_better": True,
-               "scaling": "weak", "vs_baseline": None, "dtype": args.prec, "data": "synthetic",
+               "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.prec == "f32" else "f64", "data": "synthetic",
                "config": dict(workload_config(cfg, args.workload, prec, recon),
                               l2="working set (2 link sets + %d vectors = %.0f MB) larger than the 126 MB L2; no flush"
                                  % (2 * nshift + 4, (ctx.gauge_packed_bytes(prec, recon) + (2 * nshift + 4) * vb) / 1e6)),
@@ -487,7 +490,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
-    ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32", "f64split"],
+                    help="f64split = N3: fp64 vectors on split-double (b + c) links")
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-block", action="store_true", help="skip the N1 multi-source measurements")

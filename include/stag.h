@@ -72,7 +72,13 @@ enum {
     STAG_ERR_NOTCONV = -5,      /* maxiter reached (or fp32 stagnation); outputs still written  */
     STAG_ERR_BREAKDOWN = -6     /* <p,Ap> <= 0 or NaN inside CG                                 */
 };
-enum { STAG_F64 = 0, STAG_F32 = 1 };
+/* STAG_F64_SPLIT (N3): fp64 vectors and arithmetic on links stored as TWO fp32
+ * numbers per real, b = (float)a and c = (float)(a - (double)b); the kernels rebuild a' = b + c
+ * (48 significant bits).  The first stag_gauge_packed_bytes(ctx, STAG_F32, recon) bytes of a split
+ * buffer ARE the STAG_F32 packed format (the b planes), so the same resident buffer also serves
+ * every prec = STAG_F32 call.  Wherever a `prec` sizes or converts a VECTOR, STAG_F64_SPLIT means
+ * STAG_F64.  Not accepted by the *_block calls (STAG_ERR_UNSUPPORTED). */
+enum { STAG_F64 = 0, STAG_F32 = 1, STAG_F64_SPLIT = 2 };
 enum { STAG_RECON18 = 18, STAG_RECON12 = 12 };
 
 typedef struct stag_ctx stag_ctx;

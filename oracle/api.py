@@ -165,3 +165,18 @@ def dense_solve(A, sigma: float, b) -> np.ndarray:
     if rc:
         raise ValueError("oracle_dense_solve rc=%d" % rc)
     return x
+
+
+def split_double(a: np.ndarray) -> np.ndarray:
+    """N3: "write a double precision number a by using two single precision numbers b
+    and c": b = (float)a, c = (float)(a - (double)b), and "reconstruct the double
+    precision number a to be used in calculations" = (double)b + (double)c.  Returns that reconstruction
+    a' (same shape; complex arrays are split component-wise).  b + c carries 48 significant bits, so
+    |a' - a| <= 2^-48 |a| (pin: tests/test_oracle_pins.py::test_N3_split_double)."""
+    a = np.asarray(a)
+    if np.iscomplexobj(a):
+        return split_double(a.real) + 1j * split_double(a.imag)
+    a = a.astype(np.float64)
+    b = a.astype(np.float32)
+    c = (a - b.astype(np.float64)).astype(np.float32)
+    return b.astype(np.float64) + c.astype(np.float64)

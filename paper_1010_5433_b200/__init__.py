@@ -6,6 +6,6 @@ PyTorch is used for device memory and streams.  There is no CPU fallback: import
 binding without a built library raises.
 """
 from .binding import (  # noqa: F401
-    F64, F32, RECON18, RECON12, MAX_SHIFTS, MAX_RHS, OK, ERR_BADARG, ERR_UNSUPPORTED, ERR_CUDA,
+    F64, F32, F64_SPLIT, RECON18, RECON12, MAX_SHIFTS, MAX_RHS, OK, ERR_BADARG, ERR_UNSUPPORTED, ERR_CUDA,
     ERR_NOT_SU3, ERR_NOTCONV, ERR_BREAKDOWN, StagError, CgInfo, Stag, lib, strerror, SYMBOLS,
 )

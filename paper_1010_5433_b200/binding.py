@@ -10,7 +10,7 @@ import torch
 HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(HERE, "libstag_b200.so")
 
-F64, F32 = 0, 1
+F64, F32, F64_SPLIT = 0, 1, 2      # F64_SPLIT (N3): split-double links, fp64 vectors
 RECON18, RECON12 = 18, 12
 MAX_SHIFTS = 32
 MAX_RHS = 4

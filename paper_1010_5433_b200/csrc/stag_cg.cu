@@ -371,7 +371,7 @@ extern "C" int stag_mshift_cg(const stag_ctx *ctx, const void *packed, int prec,
     if (!(mass * mass + smin > 0.0)) return STAG_ERR_BADARG;
     if (((uintptr_t)workspace & 255) != 0) return STAG_ERR_BADARG;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (prec == STAG_F64)
+    if (prec != STAG_F32)
         return run_cg<double>(ctx, packed, prec, recon, b_even, mass, nshift, host_shifts,
                               host_residues, residue0, stop, maxiter, x_even, y_even, workspace,
                               info, st);

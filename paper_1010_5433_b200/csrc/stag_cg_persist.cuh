@@ -216,7 +216,7 @@ struct PersistArgs {
     int res_r, res_q, res_p;   // which slices are resident in shared memory
 };
 
-template <typename T, int RECON, int NT, int R>
+template <typename T, int RECON, int NT, int R, bool SPLIT = false>
 __global__ void __launch_bounds__(NT, 1)
 cg_persistent_kernel(const Geom g, const PersistArgs a) {
     extern __shared__ __align__(16) unsigned char dyn[];
@@ -333,7 +333,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
         // phase A (a2): w = D_oe p_base on this CTA's odd sites
         for (int ls = tid; ls < ns; ls += NT) {
             T acc[R][6];
-            dslash_site_multi<T, RECON, R, false>(g, a.W, pin, mask, 1, e0 + ls, acc);
+            dslash_site_multi<T, RECON, R, false, SPLIT>(g, a.W, pin, mask, 1, e0 + ls, acc);
 #pragma unroll
             for (int r = 0; r < R; ++r)
                 if (R == 1 || ((mask >> r) & 1u)) store_vec(wout[r], Vh, e0 + ls, acc[r]);
@@ -349,7 +349,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             for (int ls = tid; ls < ns; ls += NT) {
                 const int e = e0 + ls;
                 T acc[R][6];
-                dslash_site_multi<T, RECON, R, false>(g, a.W, win, mask, 0, e, acc);
+                dslash_site_multi<T, RECON, R, false, SPLIT>(g, a.W, win, mask, 0, e, acc);
 #pragma unroll
                 for (int r = 0; r < R; ++r)
                     if (R == 1 || ((mask >> r) & 1u)) {
@@ -573,7 +573,7 @@ inline int sites_per_cta(int Vh, int grid) {
     return (s + 31) & ~31;
 }
 
-template <typename T, int RECON, int NT, int R>
+template <typename T, int RECON, int NT, int R, bool SPLIT = false>
 int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t st) {
     const Geom &g = ctx->g;
     int grid = ctx->num_sms;
@@ -586,7 +586,7 @@ int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t
     const int fit = (int)(kMaxDynSmem / slice);
     a.res_r = fit >= 1; a.res_q = fit >= 2; a.res_p = fit >= 3;
     const size_t smem = slice * (size_t)(a.res_r + a.res_q + a.res_p);
-    auto kern = cg_persistent_kernel<T, RECON, NT, R>;
+    auto kern = cg_persistent_kernel<T, RECON, NT, R, SPLIT>;
     STAG_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     STAG_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
@@ -600,6 +600,9 @@ int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t
 // one explicit-instantiation translation unit per R (parallel compilation)
 template <int R>
 int cg_persistent_launch_r(const stag_ctx *ctx, int prec, int recon, const PersistArgs &a, cudaStream_t st);
+
+// N3: single source on split-double links (stag_cg_persist_split.cu)
+int cg_persistent_launch_split(const stag_ctx *ctx, int recon, const PersistArgs &a, cudaStream_t st);
 
 #define STAG_DEFINE_PERSIST_R(RR)                                                                       \
     template <>                                                                                         \

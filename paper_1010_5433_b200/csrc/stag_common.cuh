@@ -84,14 +84,16 @@ namespace stag {
         if (e__ != cudaSuccess) return STAG_ERR_CUDA;       \
     } while (0)
 
-inline bool valid_prec(int p) { return p == STAG_F64 || p == STAG_F32; }
+inline bool valid_prec(int p) { return p == STAG_F64 || p == STAG_F32 || p == STAG_F64_SPLIT; }
+// precision of the colour vectors that go with a gauge format (split-double links carry fp64 vectors)
+inline int vec_prec(int p) { return p == STAG_F32 ? STAG_F32 : STAG_F64; }
 inline bool valid_recon(int r) { return r == STAG_RECON18 || r == STAG_RECON12; }
 
 // bytes of one link set plane group: (recon reals) * sizeof(T) per site
 inline size_t link_bytes_per_site(int prec, int recon) {
-    return (size_t)recon * (prec == STAG_F64 ? 8 : 4);
+    return (size_t)recon * (prec == STAG_F32 ? 4 : 8);   // split-double: a float b plus a float c per real
 }
-inline size_t vec_bytes_per_site(int prec) { return (size_t)6 * (prec == STAG_F64 ? 8 : 4); }
+inline size_t vec_bytes_per_site(int prec) { return (size_t)6 * (prec == STAG_F32 ? 4 : 8); }
 inline size_t align256(size_t n) { return (n + 255) & ~(size_t)255; }
 
 // ---- streaming / cached 128-bit and 64-bit loads ---------------------------------------------

@@ -18,7 +18,7 @@ namespace stag {
 template <int BLOCK, int RT>
 constexpr int min_ctas() { return RT / BLOCK > 0 ? RT / BLOCK : 1; }
 
-template <typename T, int RECON, int BLOCK, int MODE, int RT>
+template <typename T, int RECON, int BLOCK, int MODE, int RT, bool SPLIT = false>
 __global__ void __launch_bounds__(BLOCK, (min_ctas<BLOCK, RT>()))
 dslash_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ in,
               char *__restrict__ out, const int par, const char *__restrict__ p,
@@ -37,7 +37,7 @@ dslash_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__
     if (MODE == 2) c0 = (T)state->c0;
     for (int e = blockIdx.x * BLOCK + threadIdx.x; e < g.Vh; e += gridDim.x * BLOCK) {
         T acc[6];
-        dslash_site<T, RECON>(g, W, in, par, e, acc);
+        dslash_site<T, RECON, true, SPLIT>(g, W, in, par, e, acc);
         if (MODE == 2) {
             T pv[6];
             load_vec(p, g.Vh, e, pv);
@@ -140,6 +140,19 @@ static int launch_dslash(const stag_ctx *ctx, const void *packed, const void *in
     return STAG_OK;
 }
 
+// N3: split-double links, fp64 vectors.  One configuration: 128 threads, 128 registers (the fp64 default).
+template <int RECON, int MODE>
+static int launch_dslash_split(const stag_ctx *ctx, const void *packed, const void *in, void *out, int par,
+                               const void *p, CgState *state, double *partials, cudaStream_t st) {
+    const Geom &g = ctx->g;
+    const int grid = dslash_grid(ctx, 128, MODE == 2);
+    dslash_kernel<double, RECON, 128, MODE, 512, true><<<grid, 128, 0, st>>>(
+        g, static_cast<const char *>(packed), static_cast<const char *>(in), static_cast<char *>(out), par,
+        static_cast<const char *>(p), state, partials);
+    STAG_CUDA_OK(cudaGetLastError());
+    return STAG_OK;
+}
+
 template <int MODE>
 static int dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon, const void *in,
                     void *out, int par, const void *p, CgState *state, double *partials,
@@ -147,6 +160,9 @@ static int dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon
     if (!ctx || !packed || !in || !out || in == out) return STAG_ERR_BADARG;
     if (!valid_prec(prec) || !valid_recon(recon)) return STAG_ERR_BADARG;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (prec == STAG_F64_SPLIT)
+        return recon == 18 ? launch_dslash_split<18, MODE>(ctx, packed, in, out, par, p, state, partials, st)
+                           : launch_dslash_split<12, MODE>(ctx, packed, in, out, par, p, state, partials, st);
     if (prec == STAG_F64)
         return recon == 18
                    ? launch_dslash<double, 18, MODE>(ctx, packed, in, out, par, p, state, partials, st)
@@ -184,6 +200,7 @@ extern "C" int stag_dslash_block(const stag_ctx *ctx, const void *packed, int pr
     if (!ctx || !packed || !in || !out || in == out) return STAG_ERR_BADARG;
     if (!valid_prec(prec) || !valid_recon(recon) || (out_parity != 0 && out_parity != 1)) return STAG_ERR_BADARG;
     if (nrhs < 1 || nrhs > STAG_MAX_RHS) return STAG_ERR_BADARG;
+    if (prec == STAG_F64_SPLIT) return STAG_ERR_UNSUPPORTED;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (ctx->opt.dslash_pipe != 0) {
         const int rc = dslash_pipe_dispatch(ctx, packed, prec, recon, out_parity, nrhs, in, out, st);

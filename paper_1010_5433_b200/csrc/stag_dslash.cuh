@@ -106,6 +106,30 @@ __device__ __forceinline__ void load_link(const char *__restrict__ w, int Vh, in
     }
 }
 
+// N3 split-double links ("write a double precision number a by using two single
+// precision numbers b and c ... reconstruct the double precision number a to be used in
+// calculations"): wb = this direction's b planes in the fp32 packed layout, wb + c_off = its c planes.
+template <int RECON>
+__device__ __forceinline__ void load_link_split(const char *__restrict__ wb, size_t c_off, int Vh, int e,
+                                                double (&u)[18], double c3, uint64_t pol) {
+    const float4 *pb = reinterpret_cast<const float4 *>(wb) + e;
+    const float4 *pc = reinterpret_cast<const float4 *>(wb + c_off) + e;
+#pragma unroll
+    for (int k = 0; k < RECON / 4; ++k) {
+        const float4 b = ld_stream(pb + (size_t)k * Vh, pol);
+        const float4 c = ld_stream(pc + (size_t)k * Vh, pol);
+        u[4 * k] = (double)b.x + (double)c.x; u[4 * k + 1] = (double)b.y + (double)c.y;
+        u[4 * k + 2] = (double)b.z + (double)c.z; u[4 * k + 3] = (double)b.w + (double)c.w;
+    }
+    if (RECON == 18) {
+        const float2 b = ld_stream(reinterpret_cast<const float2 *>(wb + (size_t)Vh * 64) + e, pol);
+        const float2 c = ld_stream(reinterpret_cast<const float2 *>(wb + c_off + (size_t)Vh * 64) + e, pol);
+        u[16] = (double)b.x + (double)c.x; u[17] = (double)b.y + (double)c.y;
+    } else {
+        rebuild_row3(u, c3);
+    }
+}
+
 template <typename T>
 __device__ __forceinline__ void matvec_acc(const T (&u)[18], const T (&v)[6], T (&acc)[6]) {
 #pragma unroll
@@ -131,14 +155,18 @@ __device__ __host__ __forceinline__ size_t link_set_bytes(int Vh) {
 // ONE load of the 8 hopping matrices (N1: links are 92 % of the stencil's bytes;
 // the paper's multiple pseudo-fermions).  W: packed gauge base (both parities).
 // `mask` bit r = source r wanted (uniform over the CTA); the others cost nothing.
-template <typename T, int RECON, int R, bool NC = true>
+// SPLIT (T = double only): W is a split-double buffer (N3).
+template <typename T, int RECON, int R, bool NC = true, bool SPLIT = false>
 __device__ __forceinline__ void dslash_site_multi(const Geom &g, const char *__restrict__ W,
                                                   const char *const (&in)[R], unsigned mask, int par,
                                                   int e, T (&acc)[R][6]) {
+    static_assert(!SPLIT || sizeof(T) == 8, "split-double links carry fp64 vectors");
     const Site s = site_of(g, e, par);
     const int Vh = g.Vh;
     const uint64_t pol = policy_evict_first();
-    const char *wp = W + (size_t)par * 8 * link_set_bytes<T, RECON>(Vh);
+    const size_t set = SPLIT ? link_set_bytes<float, RECON>(Vh) : link_set_bytes<T, RECON>(Vh);
+    const size_t c_off = 16 * set;                       // split: the c planes follow the 16 b sets
+    const char *wp = W + (size_t)par * 8 * set;
     const int x[4] = {s.x0, s.x1, s.x2, s.x3};
     int stride = 1;
     int phase_sum = 0;
@@ -158,14 +186,16 @@ __device__ __forceinline__ void dslash_site_multi(const Geom &g, const char *__r
             c3b = (mu == 3 && x[3] == 0) ? eta : -eta;
         }
         T u[18], v[6];
-        load_link<RECON>(wp + (size_t)(2 * mu) * link_set_bytes<T, RECON>(Vh), Vh, e, u, c3f, pol);
+        if constexpr (SPLIT) load_link_split<RECON>(wp + (size_t)(2 * mu) * set, c_off, Vh, e, u, c3f, pol);
+        else load_link<RECON>(wp + (size_t)(2 * mu) * set, Vh, e, u, c3f, pol);
 #pragma unroll
         for (int r = 0; r < R; ++r)
             if (R == 1 || ((mask >> r) & 1u)) {
                 load_vec<NC>(in[r], Vh, ef, v);
                 matvec_acc(u, v, acc[r]);
             }
-        load_link<RECON>(wp + (size_t)(2 * mu + 1) * link_set_bytes<T, RECON>(Vh), Vh, e, u, c3b, pol);
+        if constexpr (SPLIT) load_link_split<RECON>(wp + (size_t)(2 * mu + 1) * set, c_off, Vh, e, u, c3b, pol);
+        else load_link<RECON>(wp + (size_t)(2 * mu + 1) * set, Vh, e, u, c3b, pol);
 #pragma unroll
         for (int r = 0; r < R; ++r)
             if (R == 1 || ((mask >> r) & 1u)) {
@@ -178,12 +208,12 @@ __device__ __forceinline__ void dslash_site_multi(const Geom &g, const char *__r
 }
 
 // single source
-template <typename T, int RECON, bool NC = true>
+template <typename T, int RECON, bool NC = true, bool SPLIT = false>
 __device__ __forceinline__ void dslash_site(const Geom &g, const char *__restrict__ W,
                                             const char *in, int par, int e, T (&acc)[6]) {
     const char *const ins[1] = {in};
     T a[1][6];
-    dslash_site_multi<T, RECON, 1, NC>(g, W, ins, 1u, par, e, a);
+    dslash_site_multi<T, RECON, 1, NC, SPLIT>(g, W, ins, 1u, par, e, a);
 #pragma unroll
     for (int i = 0; i < 6; ++i) acc[i] = a[0][i];
 }

@@ -4,6 +4,8 @@
 //   PAPER.md:109  12-real storage: "only the first two rows are stored"
 //   PAPER.md:113  b = (float)a   (fp32 copies are a round-to-nearest cast of the fp64 input)
 //   PAPER.md:119  "blocks of threads ... use contiguous regions of device memory" -> planes
+#include <type_traits>
+
 #include "stag_dslash.cuh"
 
 namespace stag {
@@ -33,7 +35,19 @@ __device__ __forceinline__ void write_planes(char *base, int Vh, int e, const do
             make_float2((float)m[N - 2], (float)m[N - 1]);
 }
 
-// blockIdx.y = p*8 + d
+// N3 split-double: b = (float)a, c = (float)(a - (double)b), each in the fp32 planes
+// layout; `base` = this (parity, direction)'s b planes, base + c_off = its c planes.
+struct SplitTag {};
+template <int N>
+__device__ __forceinline__ void write_planes_split(char *base, size_t c_off, int Vh, int e, const double (&m)[18]) {
+    double lo[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) lo[k] = m[k] - (double)(float)m[k];
+    write_planes<N>(base, Vh, e, m, 0.0f);
+    write_planes<N>(base + c_off, Vh, e, lo, 0.0f);
+}
+
+// blockIdx.y = p*8 + d.  T = double | float | SplitTag.
 template <typename T, int RECON>
 __global__ void __launch_bounds__(128)
 gauge_pack_kernel(const Geom g, const double *__restrict__ canon, char *__restrict__ packed,
@@ -103,8 +117,13 @@ gauge_pack_kernel(const Geom g, const double *__restrict__ canon, char *__restri
                 m[6 * i + 2 * j + 1] = -f * u[6 * j + 2 * i + 1];
             }
         }
-    char *base = packed + (size_t)blockIdx.y * link_set_bytes<T, RECON>(g.Vh);
-    write_planes<RECON>(base, g.Vh, e, m, T(0));
+    if constexpr (std::is_same<T, SplitTag>::value) {
+        const size_t set = link_set_bytes<float, RECON>(g.Vh);
+        write_planes_split<RECON>(packed + (size_t)blockIdx.y * set, 16 * set, g.Vh, e, m);
+    } else {
+        char *base = packed + (size_t)blockIdx.y * link_set_bytes<T, RECON>(g.Vh);
+        write_planes<RECON>(base, g.Vh, e, m, T(0));
+    }
 }
 
 template <typename T>
@@ -156,7 +175,10 @@ extern "C" int stag_gauge_pack(const stag_ctx *ctx, const double *dev_links_cano
         STAG_CUDA_OK(cudaHostGetDevicePointer((void **)&flag, ctx->pinned_flags, 0));
         ctx->pinned_flags[0] = 0;
     }
-    if (prec == STAG_F64) {
+    if (prec == STAG_F64_SPLIT) {
+        if (recon == 18) gauge_pack_kernel<SplitTag, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
+        else gauge_pack_kernel<SplitTag, 12><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
+    } else if (prec == STAG_F64) {
         if (recon == 18) gauge_pack_kernel<double, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
         else gauge_pack_kernel<double, 12><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
     } else {
@@ -177,7 +199,7 @@ extern "C" int stag_vector_pack(const stag_ctx *ctx, const double *dev_canonical
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const Geom &g = ctx->g;
     const int grid = (g.Vh + 127) / 128;
-    if (prec == STAG_F64)
+    if (prec != STAG_F32)
         vector_pack_kernel<double><<<grid, 128, 0, st>>>(g, dev_canonical, static_cast<char *>(dev_vec));
     else
         vector_pack_kernel<float><<<grid, 128, 0, st>>>(g, dev_canonical, static_cast<char *>(dev_vec));
@@ -191,7 +213,7 @@ extern "C" int stag_vector_unpack(const stag_ctx *ctx, const void *dev_vec, int 
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const Geom &g = ctx->g;
     const int grid = (g.Vh + 127) / 128;
-    if (prec == STAG_F64)
+    if (prec != STAG_F32)
         vector_unpack_kernel<double><<<grid, 128, 0, st>>>(g, static_cast<const char *>(dev_vec), dev_canonical);
     else
         vector_unpack_kernel<float><<<grid, 128, 0, st>>>(g, static_cast<const char *>(dev_vec), dev_canonical);

@@ -60,6 +60,23 @@ def test_c4_dslash_all_variants(stag, c4, prec, recon, regs):
     assert rel(ctx.download_vector(q, prec), oracle.dslash_eo(L, U, got_w)) <= TOL[prec]
 
 
+@pytest.mark.parametrize("recon", [18, 12])
+def test_c4_dslash_split_double(stag, c4, recon):
+    """N3 at full size: split-double links (b + c), fp64 vectors; within the
+    north_star's 1e-13 of the unsplit oracle (bound re-derived in tests/test_gpu_split.py)."""
+    cfg, U, srcs = c4
+    L, P = cfg["L"], stag.F64_SPLIT
+    ctx = stag.Stag(L)
+    packed = ctx.upload_gauge(U, P, recon)
+    v = srcs[1]
+    vin, w, q = ctx.upload_vector(v, P), ctx.alloc(ctx.vector_bytes(P)), ctx.alloc(ctx.vector_bytes(P))
+    ctx.dslash_oe(packed, P, recon, vin, w)
+    got_w = ctx.download_vector(w, P)
+    assert rel(got_w, oracle.dslash_oe(L, U, v)) <= 1e-13
+    ctx.dslash_eo(packed, P, recon, w, q)
+    assert rel(ctx.download_vector(q, P), oracle.dslash_eo(L, U, got_w)) <= 1e-13
+
+
 @pytest.mark.parametrize("prec,recon", [(0, 18), (0, 12), (1, 18), (1, 12)])
 @pytest.mark.parametrize("pipe", [1, 0])
 def test_c4_dslash_block_four_sources(stag, c4, prec, recon, pipe):

@@ -317,3 +317,25 @@ def test_P8_plane_wave_solution_and_partial_fraction():
     y = oracle.partial_fraction(b, residues, 0.3, res["x"])
     expect = b * (0.3 + sum(a / (lam + s) for a, s in zip(residues, SHIFTS)))
     assert rel(y, expect) < 1e-14
+
+
+# ---- N3: split-double storage, PAPER.md:111-117 ---------------------------------
+def test_N3_split_double():
+    """b = (float)a, c = (float)(a - (double)b), a' = b + c.  Pinned by (i) a worked value: a = 1/3 has
+    b = 0x3EAAAAAB = 1/3 + 2^-25/3 and c = -(1/3 + 2^-25/3) 2^-25 (float of -2^-25/3), so
+    a' = 1/3 - 2^-50/3 up to the rounding of 1/3 itself; (ii) numbers with <= 48 significant bits are
+    reproduced exactly; (iii) the 2^-48 bound on random data; (iv) a wrong formula (c dropped) fails."""
+    a = np.array([1.0 / 3.0])
+    got = oracle.split_double(a)[0]
+    assert abs(got - (1.0 / 3.0 - 2.0 ** -50 / 3.0)) <= 2.0 ** -54
+    assert got != 1.0 / 3.0 and abs(got - 1.0 / 3.0) > 2.0 ** -53
+    exact = np.array([1.0 + 2.0 ** -40, -0.5 - 2.0 ** -47, 3.0 * 2.0 ** -20 + 2.0 ** -60, 0.0, -2.0])
+    assert np.array_equal(oracle.split_double(exact), exact)
+    rng = np.random.default_rng(5)
+    r = rng.standard_normal(4096) * 10.0 ** rng.integers(-3, 3, 4096)
+    d = np.abs(oracle.split_double(r) - r)
+    assert np.all(d <= 2.0 ** -48 * np.abs(r))
+    assert np.max(d / np.abs(r)) > 2.0 ** -56                      # it is not the identity
+    assert np.max(np.abs(r.astype(np.float32).astype(np.float64) - r) / np.abs(r)) > 2.0 ** -26   # (iv)
+    z = oracle.split_double(r[:8] + 1j * r[8:16])
+    assert np.array_equal(z.real, oracle.split_double(r[:8])) and np.array_equal(z.imag, oracle.split_double(r[8:16]))
