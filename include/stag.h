@@ -188,6 +188,51 @@ int stag_mshift_cg_block(const stag_ctx *ctx, const void *packed, int prec, int 
                          void *x_even, void *y_even, void *workspace, stag_cg_info *info,
                          void *stream);
 
+/* ---- N2: mixed precision the way the paper uses it (PAPER.md:93 fp32 for the
+ * MD-force solves, fp64 for Metropolis; :127-129 a shifted solver cannot be restarted, but every
+ * single system can): an fp32 multi-shift run followed by a per-shift fp64 DEFECT-CORRECTION POLISH —
+ * ordinary CG with a non-zero start:  r_i = b - (A + sigma_i) x_i  in fp64,  (A + sigma_i) e_i = r_i
+ * by CG from zero until ||r|| <= stop ||b||,  x_i += e_i;  then the true residual is recomputed and
+ * the pass repeated (at most 3 passes) while it is above stop.  Up to STAG_MAX_RHS shifts are polished
+ * together in one persistent launch with one read of the links per Dslash (the N1 kernel, one shift per
+ * source).  Also the remedy for reading A8 (true residual slightly above stop after an fp64 multi-shift
+ * run): shifts already at or below stop are left untouched (0 iterations). */
+typedef struct stag_polish_info {
+    int passes;                              /* defect-correction passes run (0 .. 3)                     */
+    int iters[STAG_MAX_SHIFTS];              /* polish CG iterations of shift i, all passes               */
+    double resid_before[STAG_MAX_SHIFTS];    /* TRUE ||b - (A+sigma_i) x_i|| / ||b|| on entry (fp64)      */
+    double resid_after[STAG_MAX_SHIFTS];     /* ... on exit                                               */
+    int kernel_launches;
+} stag_polish_info;
+typedef struct stag_mixed_info {
+    stag_cg_info inner;                      /* the fp32 multi-shift run                                  */
+    stag_polish_info polish;
+} stag_mixed_info;
+
+/* dst = src converted between device vector formats (nvec contiguous vectors each side). */
+int stag_vector_convert(const stag_ctx *ctx, const void *src, int src_prec, void *dst, int dst_prec,
+                        int nvec, void *stream);
+
+/* Polish x_i (in/out, nshift contiguous fp64 device-format vectors) of (A + sigma_i) x_i = b in place.
+ * prec = STAG_F64 (STAG_MAX_RHS shifts per launch) or STAG_F64_SPLIT (one shift per launch); vectors fp64.
+ * Returns STAG_OK iff every resid_after <= stop, else STAG_ERR_NOTCONV (x still improved) /
+ * STAG_ERR_BREAKDOWN.  Synchronises the stream.  workspace: stag_cg_polish_workspace_bytes, 256-aligned. */
+size_t stag_cg_polish_workspace_bytes(const stag_ctx *ctx);
+int stag_cg_polish(const stag_ctx *ctx, const void *packed, int prec, int recon, const void *b_even,
+                   double mass, int nshift, const double *host_shifts, double stop, int maxiter,
+                   void *x_even, void *workspace, stag_polish_info *info, void *stream);
+
+/* fp32 multi-shift CG to inner_stop (<= 0: default 1e-5) on packed_lo (STAG_F32 format — e.g. the first
+ * half of a STAG_F64_SPLIT buffer), then the polish on packed_hi (prec_hi = STAG_F64 | STAG_F64_SPLIT) to
+ * stop, then y.  b_even, x_even, y_even: fp64 device format.  The fp32 stage ending on stagnation or
+ * maxiter is not an error: the polish finishes the job.  Returns as stag_cg_polish. */
+size_t stag_mshift_cg_mixed_workspace_bytes(const stag_ctx *ctx, int nshift);
+int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, int prec_hi, int recon_hi,
+                         const void *packed_lo, int recon_lo, const void *b_even, double mass, int nshift,
+                         const double *host_shifts, const double *host_residues, double residue0,
+                         double stop, double inner_stop, int maxiter, void *x_even, void *y_even,
+                         void *workspace, stag_mixed_info *info, void *stream);
+
 /* ---- the same calls on HOST buffers in canonical fp64 format (copies inside) --------------
  * dev_scratch: stag_host_scratch_bytes(ctx, prec, nshift) bytes of device memory
  * (nshift = 0 for stag_dslash_host).  out_parity: 0 = D_eo, 1 = D_oe. */

@@ -45,6 +45,7 @@ def lib():
                                        C.c_int, _dp, _ip, _dp, _dp, _dp]
         l.oracle_partial_fraction.argtypes = [C.c_long, _dp, C.c_int, _dp, C.c_double, _dp, _dp]
         l.oracle_partial_fraction.restype = None
+        l.oracle_cg_polish.argtypes = [_ip, _dp, _dp, C.c_double, C.c_double, C.c_double, C.c_int, _dp, _ip, _dp]
         l.oracle_dense_A.argtypes = [_ip, _dp, C.c_double, _dp]
         l.oracle_dense_solve.argtypes = [C.c_long, _dp, C.c_double, _dp, _dp]
         _lib = l
@@ -132,6 +133,21 @@ def mshift_cg(L, links, b, mass: float, shifts, stop: float, maxiter: int,
         raise ValueError("oracle_mshift_cg: bad argument")
     return dict(rc=rc, iters=iters.value, x=x, zeta=zeta, r=r,
                 rr_hist=hist[: iters.value + 1] if hist is not None else None)
+
+
+def cg_polish(L, links, b, mass: float, sigma: float, x0, stop: float, maxiter: int) -> dict:
+    """N2: ordinary CG on (A + sigma) x = b from the start vector x0.  Returns dict(rc, iters, x, res0)."""
+    vh = _vh(L)
+    links = _c128(links, (2 * vh, 4, 3, 3))
+    b = _c128(b, (vh, 3))
+    x = _c128(x0, (vh, 3)).copy()
+    iters = C.c_int(0)
+    res0 = C.c_double(0.0)
+    rc = lib().oracle_cg_polish(_L(L), _d(links), _d(b), float(mass), float(sigma), float(stop), int(maxiter),
+                                _d(x), C.byref(iters), C.byref(res0))
+    if rc == -1:
+        raise ValueError("oracle_cg_polish: bad argument")
+    return dict(rc=rc, iters=iters.value, x=x, res0=res0.value)
 
 
 def partial_fraction(b, residues, residue0: float, x) -> np.ndarray:

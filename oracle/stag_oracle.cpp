@@ -26,6 +26,9 @@
 //                          Pinned by P7, P8.
 //   * oracle_dense_*     — brute force for tiny lattices (north_star: "dense brute-force
 //                          linear solves on 2^4 and 4^4 lattices for every shift").
+//   * oracle_cg_polish   — N2: textbook CG for ONE shifted system from a non-zero
+//                          start vector.  Pinned by P9 (dense solves; zero start = oracle_mshift_cg
+//                          with one shift, iterate for iterate; exact start = 0 iterations).
 //   * oracle_partial_fraction — y = residue0*b + sum_i residues[i]*x_i.
 //
 // No blocking, fusion, tables or reordering: loops over sites, arithmetic neighbours.
@@ -214,6 +217,46 @@ int oracle_mshift_cg(const int *L, const double *links, const double *b, double 
     if (iters_out) *iters_out = iters;
     if (zeta_out) for (int i = 0; i < nshift; ++i) zeta_out[i] = zeta[i];
     if (r_out) std::memcpy(r_out, r.data(), sizeof(double) * n);
+    return rc;
+}
+
+// N2 polish: the shifted solver must start from zero, but ONE
+// system (A + sigma) x = b may start anywhere — "ordinary CG with a non-zero start", the textbook
+// algorithm written out:
+//   r = b - (A + sigma) x ; p = r ; rr = <r,r>
+//   while sqrt(rr / <b,b>) > stop:  q = (A + sigma) p ; alpha = rr / <p,q> ; x += alpha p ;
+//                                   r -= alpha q ; beta = rr_new / rr ; p = r + beta p
+// x: in = start vector, out = polished solution.  res0_out: true relative residual of the start.
+// returns 0 converged (possibly after 0 iterations), -5 maxiter, -6 breakdown, -1 bad argument.
+int oracle_cg_polish(const int *L, const double *links, const double *b, double mass, double sigma,
+                     double stop, int maxiter, double *x, int *iters_out, double *res0_out) {
+    if (stop <= 0.0 || maxiter < 0 || mass * mass + sigma <= 0.0) return -1;
+    const long n = vol(L) / 2 * 6;
+    std::vector<double> r(n), p(n), q(n), tmp(n);
+    if (oracle_apply_A(L, links, mass, sigma, x, q.data(), tmp.data())) return -1;
+    for (long k = 0; k < n; ++k) r[k] = b[k] - q[k];
+    p = r;
+    const double bb = re_dot(b, b, n);
+    double rr = re_dot(r.data(), r.data(), n);
+    if (res0_out) *res0_out = bb > 0.0 ? std::sqrt(rr / bb) : 0.0;
+    int iters = 0, rc = -5;
+    if (bb == 0.0 || std::sqrt(rr / bb) <= stop) rc = 0;
+    else
+        for (int it = 1; it <= maxiter; ++it) {
+            oracle_apply_A(L, links, mass, sigma, p.data(), q.data(), tmp.data());
+            const double pq = re_dot(p.data(), q.data(), n);
+            const double alpha = rr / pq;
+            if (!(pq > 0.0) || !std::isfinite(alpha)) { rc = -6; break; }
+            for (long k = 0; k < n; ++k) x[k] += alpha * p[k];
+            for (long k = 0; k < n; ++k) r[k] -= alpha * q[k];
+            const double rr_new = re_dot(r.data(), r.data(), n);
+            const double beta = rr_new / rr;
+            for (long k = 0; k < n; ++k) p[k] = r[k] + beta * p[k];
+            rr = rr_new;
+            iters = it;
+            if (std::sqrt(rr / bb) <= stop) { rc = 0; break; }
+        }
+    if (iters_out) *iters_out = iters;
     return rc;
 }
 

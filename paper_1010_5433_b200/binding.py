@@ -24,6 +24,8 @@ SYMBOLS = [
     "stag_gauge_load", "stag_gauge_pack", "stag_vector_pack", "stag_vector_unpack",
     "stag_dslash_eo", "stag_dslash_oe", "stag_mshift_cg", "stag_dslash_host", "stag_mshift_cg_host",
     "stag_dslash_block", "stag_cg_block_workspace_bytes", "stag_mshift_cg_block",
+    "stag_vector_convert", "stag_cg_polish_workspace_bytes", "stag_cg_polish",
+    "stag_mshift_cg_mixed_workspace_bytes", "stag_mshift_cg_mixed",
 ]
 
 
@@ -38,6 +40,23 @@ class CgInfo(C.Structure):
                     stagnated=bool(self.stagnated), bnorm2=self.bnorm2, rnorm2=self.rnorm2,
                     resid_iter=list(self.resid_iter[:nshift]), iters_shift=list(self.iters_shift[:nshift]),
                     kernel_launches=self.kernel_launches)
+
+
+class PolishInfo(C.Structure):
+    _fields_ = [("passes", C.c_int), ("iters", C.c_int * MAX_SHIFTS), ("resid_before", C.c_double * MAX_SHIFTS),
+                ("resid_after", C.c_double * MAX_SHIFTS), ("kernel_launches", C.c_int)]
+
+    def as_dict(self, nshift: int) -> dict:
+        return dict(passes=self.passes, iters=list(self.iters[:nshift]),
+                    resid_before=list(self.resid_before[:nshift]), resid_after=list(self.resid_after[:nshift]),
+                    kernel_launches=self.kernel_launches)
+
+
+class MixedInfo(C.Structure):
+    _fields_ = [("inner", CgInfo), ("polish", PolishInfo)]
+
+    def as_dict(self, nshift: int) -> dict:
+        return dict(inner=self.inner.as_dict(nshift), polish=self.polish.as_dict(nshift))
 
 
 class StagError(RuntimeError):
@@ -85,6 +104,16 @@ def lib() -> C.CDLL:
                                        C.c_double, C.c_double, C.c_int, _vp, _vp, _vp, C.POINTER(CgInfo), _vp]
     l.stag_mshift_cg.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
                                  C.c_double, C.c_double, C.c_int, _vp, _vp, _vp, C.POINTER(CgInfo), _vp]
+    l.stag_vector_convert.argtypes = [_vp, _vp, C.c_int, _vp, C.c_int, C.c_int, _vp]
+    l.stag_cg_polish_workspace_bytes.argtypes = [_vp]
+    l.stag_cg_polish_workspace_bytes.restype = _sz
+    l.stag_cg_polish.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_int, _dp, C.c_double, C.c_int,
+                                 _vp, _vp, C.POINTER(PolishInfo), _vp]
+    l.stag_mshift_cg_mixed_workspace_bytes.argtypes = [_vp, C.c_int]
+    l.stag_mshift_cg_mixed_workspace_bytes.restype = _sz
+    l.stag_mshift_cg_mixed.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
+                                       C.c_double, C.c_double, C.c_double, C.c_int, _vp, _vp, _vp,
+                                       C.POINTER(MixedInfo), _vp]
     l.stag_dslash_host.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp]
     l.stag_mshift_cg_host.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
                                       C.c_double, C.c_double, C.c_int, _vp, _vp, _vp, C.POINTER(CgInfo), _vp]
@@ -239,6 +268,44 @@ class Stag:
         if check and rc not in (OK, ERR_NOTCONV, ERR_BREAKDOWN):
             raise StagError(rc, "stag_mshift_cg_block")
         return rc, [infos[s].as_dict(n) for s in range(int(nrhs))]
+
+    # ---- N2: mixed precision (fp32 multi-shift + per-shift fp64 polish)
+    def vector_convert(self, src, src_prec, dst, dst_prec, nvec=1, stream=None):
+        rc = lib().stag_vector_convert(self._h, _ptr(src), src_prec, _ptr(dst), dst_prec, int(nvec), _stream(stream))
+        if rc:
+            raise StagError(rc, "stag_vector_convert")
+
+    def cg_polish_workspace_bytes(self): return lib().stag_cg_polish_workspace_bytes(self._h)
+    def mshift_cg_mixed_workspace_bytes(self, nshift): return lib().stag_mshift_cg_mixed_workspace_bytes(self._h, nshift)
+
+    def cg_polish(self, packed, prec, recon, b_even, mass, shifts, stop, maxiter, x_even, workspace, stream=None,
+                  check=True):
+        """Returns (rc, info dict); x_even is polished in place."""
+        sh = _darr(shifts)
+        info = PolishInfo()
+        n = sh[1].size
+        rc = lib().stag_cg_polish(self._h, _ptr(packed), prec, recon, _ptr(b_even), float(mass), n, sh[0],
+                                  float(stop), int(maxiter), _ptr(x_even), _ptr(workspace), C.byref(info),
+                                  _stream(stream))
+        if check and rc not in (OK, ERR_NOTCONV, ERR_BREAKDOWN):
+            raise StagError(rc, "stag_cg_polish")
+        return rc, info.as_dict(n)
+
+    def mshift_cg_mixed(self, packed_hi, prec_hi, recon_hi, packed_lo, recon_lo, b_even, mass, shifts, stop,
+                        maxiter, x_even, workspace, inner_stop=0.0, residues=None, residue0=0.0, y_even=None,
+                        stream=None, check=True):
+        sh = _darr(shifts)
+        rs = _darr(residues)
+        info = MixedInfo()
+        n = sh[1].size
+        rc = lib().stag_mshift_cg_mixed(self._h, _ptr(packed_hi), prec_hi, recon_hi, _ptr(packed_lo), recon_lo,
+                                        _ptr(b_even), float(mass), n, sh[0], rs[0] if rs else None,
+                                        float(residue0), float(stop), float(inner_stop), int(maxiter),
+                                        _ptr(x_even), _ptr(y_even), _ptr(workspace), C.byref(info),
+                                        _stream(stream))
+        if check and rc not in (OK, ERR_NOTCONV, ERR_BREAKDOWN):
+            raise StagError(rc, "stag_mshift_cg_mixed")
+        return rc, info.as_dict(n)
 
     # ---- host-buffer variants
     def dslash_host(self, packed, prec, recon, out_parity, host_in, host_out, dev_scratch, stream=None):

@@ -30,6 +30,7 @@ struct CgState {
     int iter;
     int done;               // 0 running | 1 finishing (x update of this iteration pending) | 2 over
     int converged, breakdown, stagnated, since_best;
+    int zero_ok;            // N2 polish: stop >= 1 means "the zero start is good enough": 0 iterations
     unsigned int ticket;    // last-block detection for the grid-wide reductions
 };
 
@@ -132,6 +133,15 @@ int dslash_eo_fused_dispatch(const stag_ctx *ctx, const void *packed, int prec, 
 // D_oe inside CG: same kernel as stag_dslash_oe but returns at once when state->done != 0.
 int dslash_oe_cg_dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon,
                           const void *p_even, void *w_odd, CgState *state, void *stream);
+
+// implemented in stag_cg_persist.cu: nrhs independent sources in one persistent launch.  src_sigma /
+// src_stop (nullable): N2 polish — nshift must be 1 and source s solves (A + src_sigma[s]) e = b_s to
+// src_stop[s]; a source whose src_stop[s] >= 1 returns e = 0 after 0 iterations.
+int block_solve(const stag_ctx *ctx, const void *packed, int prec, int recon, int nrhs, const void *b_even,
+                double mass, int nshift, const double *host_shifts, const double *src_sigma,
+                const double *src_stop, const double *host_residues, double residue0, double stop,
+                int maxiter, void *x_even, void *y_even, void *workspace, stag_cg_info *info,
+                cudaStream_t st);
 
 // implemented in stag_cg_persist.cu: the whole solve as one cooperative kernel (small lattices)
 bool cg_persistent_fits(const stag_ctx *ctx, int prec);

@@ -83,14 +83,26 @@ extern "C" int stag_mshift_cg_block(const stag_ctx *ctx, const void *packed, int
     if (prec == STAG_F64_SPLIT) return STAG_ERR_UNSUPPORTED;
     if (nshift < 1 || nshift > STAG_MAX_SHIFTS || !(stop > 0.0) || maxiter < 0) return STAG_ERR_BADARG;
     if (y_even && !host_residues) return STAG_ERR_BADARG;
-    int base = 0;
+    double smin = host_shifts[0];
     for (int i = 0; i < nshift; ++i) {
         if (!(host_shifts[i] >= 0.0)) return STAG_ERR_BADARG;
-        if (host_shifts[i] < host_shifts[base]) base = i;
+        if (host_shifts[i] < smin) smin = host_shifts[i];
     }
-    if (!(mass * mass + host_shifts[base] > 0.0)) return STAG_ERR_BADARG;
+    if (!(mass * mass + smin > 0.0)) return STAG_ERR_BADARG;
     if (((uintptr_t)workspace & 255) != 0) return STAG_ERR_BADARG;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    return block_solve(ctx, packed, prec, recon, nrhs, b_even, mass, nshift, host_shifts, nullptr, nullptr,
+                       host_residues, residue0, stop, maxiter, x_even, y_even, workspace, info,
+                       static_cast<cudaStream_t>(stream));
+}
+
+int stag::block_solve(const stag_ctx *ctx, const void *packed, int prec, int recon, int nrhs, const void *b_even,
+                      double mass, int nshift, const double *host_shifts, const double *src_sigma,
+                      const double *src_stop, const double *host_residues, double residue0, double stop,
+                      int maxiter, void *x_even, void *y_even, void *workspace, stag_cg_info *info,
+                      cudaStream_t st) {
+    int base = 0;
+    for (int i = 0; i < nshift; ++i)
+        if (host_shifts[i] < host_shifts[base]) base = i;
     char *ws = static_cast<char *>(workspace);
     const BlockLayout lay = block_layout(ctx, prec, nshift, nrhs);
     const size_t vbytes = (size_t)ctx->g.Vh * vec_bytes_per_site(prec);
@@ -109,9 +121,18 @@ extern "C" int stag_mshift_cg_block(const stag_ctx *ctx, const void *packed, int
     }
     h->nshift = nshift; h->base = base; h->maxiter = maxiter;
     h->freeze = ctx->opt.cg_freeze; h->fp32 = (prec == STAG_F32);
-    for (int s = 0; s < nrhs; ++s)
+    for (int s = 0; s < nrhs; ++s) {
+        if (src_sigma) {                       // N2 polish: one shift per source
+            h->c0 = mass * mass + src_sigma[s];
+            h->stop = src_stop[s];
+            h->zero_ok = 1;
+            // the pinned staging is re-used per source: wait until the previous copy has left it
+            if (s > 0) STAG_CUDA_OK(cudaStreamSynchronize(st));
+        }
         STAG_CUDA_OK(cudaMemcpyAsync(ws + lay.state + (size_t)s * lay.state_stride, h, sizeof(CgState),
                                      cudaMemcpyHostToDevice, st));
+    }
+    if (src_sigma) STAG_CUDA_OK(cudaStreamSynchronize(st));
 
     PersistArgs a;
     std::memset(&a, 0, sizeof(a));
@@ -127,7 +148,9 @@ extern "C" int stag_mshift_cg_block(const stag_ctx *ctx, const void *packed, int
     a.state_stride = lay.state_stride;
     a.partials = reinterpret_cast<double *>(ws + lay.partials);
     a.nrhs = nrhs;
-    int rc = nrhs == 1 ? cg_persistent_launch_r<1>(ctx, prec, recon, a, st)
+    if (prec == STAG_F64_SPLIT && nrhs != 1) return STAG_ERR_UNSUPPORTED;
+    int rc = prec == STAG_F64_SPLIT ? cg_persistent_launch_split(ctx, recon, a, st)
+           : nrhs == 1 ? cg_persistent_launch_r<1>(ctx, prec, recon, a, st)
            : nrhs == 2 ? cg_persistent_launch_r<2>(ctx, prec, recon, a, st)
                        : cg_persistent_launch_r<4>(ctx, prec, recon, a, st);
     if (rc) { cudaGetLastError(); return rc; }

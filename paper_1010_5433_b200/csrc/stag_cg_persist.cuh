@@ -133,6 +133,8 @@ struct Scalars {
     int active[STAG_MAX_SHIFTS], iters_shift[STAG_MAX_SHIFTS];
     double bb, rr, alpha, alpha_old, beta_old, best_rr, pq;
     T a_base, z_base, b_base;
+    T c0;                    // m^2 + sigma_0 of THIS source (N2: the polish solves one shift per source)
+    double stop;             // on sqrt(rr/bb) of this source
     int nlive, iter, done, converged, breakdown, stagnated, since_best;
     // done: 0 running | 1 this iteration's x/p update is the last | 2 over
 };
@@ -235,8 +237,6 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
     CgState *st = reinterpret_cast<CgState *>(reinterpret_cast<char *>(a.state) + (size_t)rhs * a.state_stride);
     const int nshift = a.state->nshift, base = a.state->base, maxiter = a.state->maxiter;   // same for every source
     const int freeze = a.state->freeze, fp32 = a.state->fp32;
-    const double stop = a.state->stop;
-    const T c0 = (T)a.state->c0;
 
     const char *b_r = a.b + (size_t)rhs * a.b_stride;
     char *p_r = a.p + (size_t)rhs * nshift * a.p_stride;
@@ -296,11 +296,14 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
         const double bb = grid_total(part_rr + (size_t)s * G, G);
         if ((tid & 31) == 0) {
             Scalars<T> &c = sc[s];
+            const CgState *ss = reinterpret_cast<const CgState *>(reinterpret_cast<const char *>(a.state) + (size_t)min(s, a.nrhs - 1) * a.state_stride);
+            c.c0 = (T)ss->c0; c.stop = ss->stop;
             c.bb = bb; c.rr = bb; c.best_rr = bb; c.alpha = 0.0; c.alpha_old = 1.0; c.beta_old = 0.0;
             c.pq = 0.0; c.iter = 0; c.done = 0; c.converged = 0; c.breakdown = 0; c.stagnated = 0;
             c.since_best = 0; c.nlive = 0;
             if (s >= a.nrhs) c.done = 2;
             else if (!(bb > 0.0)) { c.converged = (bb == 0.0); c.breakdown = !(bb == 0.0); c.done = 2; }
+            else if (ss->zero_ok && ss->stop >= 1.0) { c.converged = 1; c.done = 2; }   // polish: x = 0 already meets it
             else if (maxiter <= 0) c.done = 2;
         }
     }
@@ -344,8 +347,9 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
         // phase B (a3): q = c0 p - D_eo w, partial Re<p,q>
         {
             double dot[R];
+            T c0[R];
 #pragma unroll
-            for (int r = 0; r < R; ++r) dot[r] = 0.0;
+            for (int r = 0; r < R; ++r) { dot[r] = 0.0; c0[r] = sc[r].c0; }
             for (int ls = tid; ls < ns; ls += NT) {
                 const int e = e0 + ls;
                 T acc[R][6];
@@ -357,7 +361,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                         p_s.load(r * S + ls, r, Vh, e, pv);
 #pragma unroll
                         for (int k = 0; k < 6; ++k) {
-                            acc[r][k] = c0 * pv[k] - acc[r][k];
+                            acc[r][k] = c0[r] * pv[k] - acc[r][k];
                             dot[r] += (double)pv[k] * (double)acc[r][k];
                         }
                         q_s.store(r * S + ls, r, Vh, e, acc[r]);
@@ -435,7 +439,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                         if (c.active[i] == 1) {
                             c.resid[i] = z * rel;
                             c.iters_shift[i] = iter;
-                            if (freeze && i != base && z * rel <= 0.1 * stop) c.active[i] = 2;
+                            if (freeze && i != base && z * rel <= 0.1 * c.stop) c.active[i] = 2;
                         }
                     }
                 }
@@ -455,7 +459,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                     c.rr = rr_new;
                     c.iter = iter;
                     int done = 0;
-                    if (rel <= stop) { c.converged = 1; done = 1; }
+                    if (rel <= c.stop) { c.converged = 1; done = 1; }
                     else if (iter >= maxiter) done = 1;
                     else if (!(rr_new == rr_new)) { c.breakdown = 1; done = 1; }
                     else if (fp32) {                                     // reading A9

@@ -72,7 +72,7 @@ struct stag_ctx {
     stag::Options opt;
     int device;
     int num_sms;
-    int *pinned_flags;   // small pinned (mapped) host buffer: status words, convergence polls
+    int *pinned_flags;   // 512 B pinned (mapped) host buffer: status words, convergence polls; bytes 128.. = 16 doubles (N2 norms)
     void *pinned_info;   // pinned staging for the CG state upload / read-back (one CgState)
 };
 

@@ -37,7 +37,7 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
     c->opt.cg_persistent_threads = 0;
     if (cudaGetDevice(&c->device) != cudaSuccess ||
         cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess ||
-        cudaHostAlloc((void **)&c->pinned_flags, 64, cudaHostAllocMapped) != cudaSuccess ||
+        cudaHostAlloc((void **)&c->pinned_flags, 512, cudaHostAllocMapped) != cudaSuccess ||
         cudaHostAlloc(&c->pinned_info, sizeof(CgState), cudaHostAllocDefault) != cudaSuccess) {
         cudaGetLastError();
         stag_ctx_destroy(c);

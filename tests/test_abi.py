@@ -49,10 +49,12 @@ def test_strerror_and_info_struct_layout(so_path, tmp_path):
     assert "converge" in stag.strerror(stag.ERR_NOTCONV)
     # sizeof(stag_cg_info) as the C compiler sees it == ctypes mirror
     src = tmp_path / "s.c"
-    src.write_text('#include <stdio.h>\n#include "stag.h"\nint main(void){printf("%zu", sizeof(stag_cg_info));return 0;}\n')
+    src.write_text('#include <stdio.h>\n#include "stag.h"\nint main(void){printf("%zu %zu %zu", sizeof(stag_cg_info), '
+                   'sizeof(stag_polish_info), sizeof(stag_mixed_info));return 0;}\n')
     exe = tmp_path / "s"
     subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
-    assert int(subprocess.check_output([str(exe)])) == ctypes.sizeof(stag.CgInfo)
+    sizes = [int(v) for v in subprocess.check_output([str(exe)]).split()]
+    assert sizes == [ctypes.sizeof(stag.CgInfo), ctypes.sizeof(stag.PolishInfo), ctypes.sizeof(stag.MixedInfo)]
 
 
 def test_no_cpu_fallback_without_gpu():

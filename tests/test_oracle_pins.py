@@ -339,3 +339,48 @@ def test_N3_split_double():
     assert np.max(np.abs(r.astype(np.float32).astype(np.float64) - r) / np.abs(r)) > 2.0 ** -26   # (iv)
     z = oracle.split_double(r[:8] + 1j * r[8:16])
     assert np.array_equal(z.real, oracle.split_double(r[:8])) and np.array_equal(z.imag, oracle.split_double(r[8:16]))
+
+
+# ---- N2: polish = ordinary CG from a non-zero start, PAPER.md:125-129 -------------
+def _fp32_like(x, seed):
+    """a start vector of fp32 quality: the solution rounded to fp32 plus 1e-6 relative noise"""
+    rng = np.random.default_rng(seed)
+    x32 = x.astype(np.complex64).astype(np.complex128)
+    return x32 + 1e-6 * np.linalg.norm(x) / np.sqrt(x.size) * (rng.standard_normal(x.shape) + 1j * rng.standard_normal(x.shape))
+
+
+@pytest.mark.parametrize("L", [(2, 2, 2, 2), (4, 4, 4, 4)])
+def test_P9_polish_reaches_the_dense_solution(L):
+    U, b, m = si.links_haar(L, 41), si.source_gaussian(L, 41), 0.1
+    A = oracle.dense_A(L, U, m)
+    for sigma in (0.0, 0.04, 0.64):
+        xd = oracle.dense_solve(A, sigma, b).reshape(-1, 3)
+        x0 = _fp32_like(xd, 3)
+        res = oracle.cg_polish(L, U, b, m, sigma, x0, 1e-12, 2000)
+        assert res["rc"] == 0 and res["iters"] > 0
+        assert 1e-8 < res["res0"] < 1e-4                       # an fp32-quality start
+        assert abs(res["res0"] - np.linalg.norm(b - oracle.apply_A(L, U, m, sigma, x0)) / np.linalg.norm(b)) <= 1e-12
+        assert rel(res["x"], xd) <= 1e-10
+        assert np.linalg.norm(b - oracle.apply_A(L, U, m, sigma, res["x"])) / np.linalg.norm(b) <= 1e-12
+        full = oracle.cg_polish(L, U, b, m, sigma, np.zeros_like(b), 1e-12, 2000)
+        assert res["iters"] < full["iters"]                    # a good start saves iterations
+
+
+def test_P9_polish_from_zero_is_the_single_shift_solver():
+    L = (4, 4, 4, 4)
+    U, b, m, sigma = si.links_haar(L, 42), si.source_gaussian(L, 42), 0.1, 0.02
+    a = oracle.cg_polish(L, U, b, m, sigma, np.zeros_like(b), 1e-10, 2000)
+    c = oracle.mshift_cg(L, U, b, m, [sigma], 1e-10, 2000)
+    assert a["rc"] == 0 and a["iters"] == c["iters"] and a["res0"] == 1.0
+    assert rel(a["x"], c["x"][0]) <= 1e-14
+
+
+def test_P9_polish_of_the_exact_solution_and_bad_args():
+    L = (2, 2, 2, 2)
+    U, b, m = si.links_haar(L, 43), si.source_gaussian(L, 43), 0.2
+    xd = oracle.dense_solve(oracle.dense_A(L, U, m), 0.3, b).reshape(-1, 3)
+    res = oracle.cg_polish(L, U, b, m, 0.3, xd, 1e-10, 100)
+    assert res["rc"] == 0 and res["iters"] == 0 and np.array_equal(res["x"], xd)
+    assert oracle.cg_polish(L, U, b, m, 0.3, np.zeros_like(b), 1e-30, 3)["rc"] == -5
+    with pytest.raises(ValueError):
+        oracle.cg_polish(L, U, b, m, 0.3, xd, 0.0, 10)
