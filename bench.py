@@ -283,6 +283,35 @@ def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
     return out
 
 
+def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
+    """N2 + N3: stag_mshift_cg_mixed on ONE resident split-double buffer (fp32 stage reads its b planes, the
+    fp64 polish reads b + c), same source, shifts and stop as the fp64 step; second of two runs timed."""
+    n = len(cfg["shifts"])
+    split = ctx.upload_gauge(U, stag.F64_SPLIT, 18)
+    p64 = ctx.upload_gauge(U, stag.F64, 18)
+    vb = ctx.vector_bytes(stag.F64)
+    b = ctx.upload_vector(srcs[0], stag.F64)
+    x = ctx.alloc(n * vb)
+    ws = ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(n))
+    out = {}
+    for name, hi, prec_hi, lo in (("split_buffer", split, stag.F64_SPLIT, split), ("f64_polish_f32_inner", p64, stag.F64, split)):
+        for _ in range(2):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            rc, info = ctx.mshift_cg_mixed(hi, prec_hi, 18, lo, 18, b, cfg["mass"], cfg["shifts"], cfg["stops"][0],
+                                           100000, x, ws)
+            e1.record()
+            torch.cuda.synchronize()
+        secs = e0.elapsed_time(e1) * 1e-3
+        out[name] = {"rc": rc, "s_per_solve": secs, "vs_fp64_multishift": fp64_s_per_solve / secs,
+                     "inner_fp32_iters": info["inner"]["iters"], "polish_iters": info["polish"]["iters"],
+                     "polish_passes": info["polish"]["passes"],
+                     "true_resid_after_fp32": max(info["polish"]["resid_before"]),
+                     "true_resid_final": max(info["polish"]["resid_after"]),
+                     "kernel_launches": info["inner"]["kernel_launches"] + info["polish"]["kernel_launches"]}
+    return out
+
+
 def dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, pack_ms, gen_s):
     """--dslash-only: the SURVEY.md §8(d) Dslash bandwidth sweep alone (no CG), one JSON line."""
     peak, peak_src = measured_peak_gbs()
@@ -451,6 +480,11 @@ def run_ours(args):
     if rank == 0 and not args.no_block and len(srcs) >= 2 and prec != stag.F64_SPLIT:
         block = measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak)
 
+    # ---- N2/N3: fp32 multi-shift + fp64 polish on one split-double buffer -----------------------------
+    mixed = None
+    if rank == 0 and not args.no_block and prec == stag.F64:
+        mixed = measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, secs / args.steps)
+
     # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -472,7 +506,7 @@ def run_ours(args):
                       "gbs_algorithmic": cg_gbs, "pct_of_8tbs": 100 * cg_gbs / NOMINAL_HBM_GBS,
                       "pct_of_measured": 100 * cg_gbs / peak, "solves": nsolves,
                       "iters_shift_first_solve": infos[0]["iters_shift"]},
-               "dslash": dslash, "block": block, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
+               "dslash": dslash, "block": block, "mixed": mixed, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
                "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
                        "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": te_s / e2e_steps,
                        "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},
@@ -494,7 +528,7 @@ def main():
                     help="f64split = N3: fp64 vectors on split-double (b + c) links")
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-block", action="store_true", help="skip the N1 multi-source measurements")
+    ap.add_argument("--no-block", action="store_true", help="skip the N1 multi-source and N2/N3 mixed-precision measurements")
     ap.add_argument("--ref-seconds", type=float, default=150.0,
                     help="--impl reference: total oracle time budget over all steps")
     ap.add_argument("--dslash-only", action="store_true", help="Dslash bandwidth sweep only (no CG)")

@@ -214,7 +214,7 @@ int stag_vector_convert(const stag_ctx *ctx, const void *src, int src_prec, void
                         int nvec, void *stream);
 
 /* Polish x_i (in/out, nshift contiguous fp64 device-format vectors) of (A + sigma_i) x_i = b in place.
- * prec = STAG_F64 (STAG_MAX_RHS shifts per launch) or STAG_F64_SPLIT (one shift per launch); vectors fp64.
+ * prec = STAG_F64 or STAG_F64_SPLIT (STAG_MAX_RHS shifts per persistent launch either way); vectors fp64.
  * Returns STAG_OK iff every resid_after <= stop, else STAG_ERR_NOTCONV (x still improved) /
  * STAG_ERR_BREAKDOWN.  Synchronises the stream.  workspace: stag_cg_polish_workspace_bytes, 256-aligned. */
 size_t stag_cg_polish_workspace_bytes(const stag_ctx *ctx);
@@ -232,6 +232,23 @@ int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, int prec_hi
                          const double *host_shifts, const double *host_residues, double residue0,
                          double stop, double inner_stop, int maxiter, void *x_even, void *y_even,
                          void *workspace, stag_mixed_info *info, void *stream);
+
+/* ---- N4: the first consumer of the x_i — the fermion force of the rational
+ * pseudo-fermion action S[U] = b^dag (residue0 + sum_i residues_i (A + sigma_i)^-1) b,
+ * one thread per link.  With X_i = x_i on even sites and D_oe x_i on odd sites,
+ *   F_mu(z) = 2 TA( f U_mu(z) . eps(z) sum_i residues_i X_i(z+mu) X_i(z)^dag ),  f = 1/2 eta_mu(z) s_mu(z),
+ *   eps = +1 / -1 on even / odd z,  TA(G) = (G - G^dag)/2 - tr(G - G^dag)/6,
+ * i.e. d/dt S[U_mu(z) -> exp(itT) U_mu(z)] at t = 0 is tr(i T F_mu(z)) for Hermitian traceless T.
+ *   x_even     nshift contiguous device-format vectors of `prec` (the output of stag_mshift_cg)
+ *   dev_force  out, fp64 [V][4][3][3][2] (site lex, mu, row, column, re/im) — the canonical link layout;
+ *              accumulate != 0 adds to it (several pseudo-fermions)
+ *   workspace  stag_force_workspace_bytes (the nshift odd vectors D_oe x_i), 256-byte aligned
+ * prec = STAG_F64 | STAG_F32 (the paper's choice for the force); outer products in prec, the
+ * 3x3 product and projection in fp64.  Asynchronous: 1 + ceil(nshift / STAG_MAX_RHS) launches, no sync. */
+size_t stag_force_workspace_bytes(const stag_ctx *ctx, int prec, int nshift);
+int stag_fermion_force(const stag_ctx *ctx, const void *packed, int prec, int recon, int nshift,
+                       const double *host_residues, const void *x_even, double *dev_force, int accumulate,
+                       void *workspace, void *stream);
 
 /* ---- the same calls on HOST buffers in canonical fp64 format (copies inside) --------------
  * dev_scratch: stag_host_scratch_bytes(ctx, prec, nshift) bytes of device memory

@@ -6,5 +6,5 @@ package; the product (paper_1010_5433_b200/) never does and shares no code with 
 """
 from .api import (  # noqa: F401
     build, lib, set_threads, dslash, dslash_eo, dslash_oe, apply_A, mshift_cg, norm2,
-    partial_fraction, dense_A, dense_solve, split_double, cg_polish,
+    partial_fraction, dense_A, dense_solve, split_double, cg_polish, fermion_force,
 )

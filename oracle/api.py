@@ -46,6 +46,7 @@ def lib():
         l.oracle_partial_fraction.argtypes = [C.c_long, _dp, C.c_int, _dp, C.c_double, _dp, _dp]
         l.oracle_partial_fraction.restype = None
         l.oracle_cg_polish.argtypes = [_ip, _dp, _dp, C.c_double, C.c_double, C.c_double, C.c_int, _dp, _ip, _dp]
+        l.oracle_fermion_force.argtypes = [_ip, _dp, C.c_int, _dp, _dp, _dp]
         l.oracle_dense_A.argtypes = [_ip, _dp, C.c_double, _dp]
         l.oracle_dense_solve.argtypes = [C.c_long, _dp, C.c_double, _dp, _dp]
         _lib = l
@@ -148,6 +149,20 @@ def cg_polish(L, links, b, mass: float, sigma: float, x0, stop: float, maxiter: 
     if rc == -1:
         raise ValueError("oracle_cg_polish: bad argument")
     return dict(rc=rc, iters=iters.value, x=x, res0=res0.value)
+
+
+def fermion_force(L, links, residues, x) -> np.ndarray:
+    """N4: F [V][4][3][3] (traceless anti-Hermitian) with d/dt S[exp(itT) U_mu(z)] = tr(i T F_mu(z)) for
+    S = b^dag (residue0 + sum_i residues_i (A+sigma_i)^-1) b and x[i] = (A+sigma_i)^-1 b."""
+    vh = _vh(L)
+    links = _c128(links, (2 * vh, 4, 3, 3))
+    res = np.ascontiguousarray(residues, dtype=np.float64)
+    x = _c128(x, (res.size, vh, 3))
+    F = np.empty((2 * vh, 4, 3, 3), dtype=np.complex128)
+    rc = lib().oracle_fermion_force(_L(L), _d(links), res.size, _d(res), _d(x), _d(F))
+    if rc:
+        raise ValueError("oracle_fermion_force rc=%d" % rc)
+    return F
 
 
 def partial_fraction(b, residues, residue0: float, x) -> np.ndarray:

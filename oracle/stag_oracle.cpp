@@ -29,6 +29,9 @@
 //   * oracle_cg_polish   — N2: textbook CG for ONE shifted system from a non-zero
 //                          start vector.  Pinned by P9 (dense solves; zero start = oracle_mshift_cg
 //                          with one shift, iterate for iterate; exact start = 0 iterations).
+//   * oracle_fermion_force — N4: derivative of the rational pseudo-fermion action on every link
+//                          (outer products of x_i and D_oe x_i).  Pinned by P10: finite differences
+//                          of the action computed from dense solves.
 //   * oracle_partial_fraction — y = residue0*b + sum_i residues[i]*x_i.
 //
 // No blocking, fusion, tables or reordering: loops over sites, arithmetic neighbours.
@@ -258,6 +261,78 @@ int oracle_cg_polish(const int *L, const double *links, const double *b, double 
         }
     if (iters_out) *iters_out = iters;
     return rc;
+}
+
+// N4 (SURVEY.md §8(f); PAPER.md:25 "fermion force", :87 "a thread ... to every link", :93): the
+// force of the rational pseudo-fermion action  S[U] = b^dag ( residue0 + sum_i residues_i (A+sigma_i)^-1 ) b
+// on every link, given the solutions x_i = (A+sigma_i)^-1 b (even sites).  The paper prints no
+// formula; this is the derivative of S written out (derivation in DESIGN.md "N4"):
+//   X_i = x_i on even sites, D_oe x_i on odd sites;  eps(z) = +1 (z even) / -1 (z odd)
+//   M_mu(z) = eps(z) sum_i residues_i X_i(z+mu) X_i(z)^dag                     (3x3 outer products)
+//   F_mu(z) = 2 f_mu(z) TA( U_mu(z) M_mu(z) ),   f = 1/2 eta_mu(z) s_mu(z)  (the hop's own factor),
+//   TA(G) = (G - G^dag)/2 - tr(G - G^dag)/6      (traceless anti-Hermitian part)
+// so that  d/dt S[ U_mu(z) -> exp(i t T) U_mu(z) ] at t = 0  equals  tr( i T F_mu(z) )  for every
+// Hermitian traceless T.  Pinned by exactly that statement with S from dense solves (P10).
+// x: double[nshift][Vh][3][2]; force out: double[V][4][3][3][2] (site lex, mu, row, col, re/im).
+int oracle_fermion_force(const int *L, const double *links, int nshift, const double *residues,
+                         const double *x, double *force) {
+    if (nshift < 1) return -1;
+    for (int mu = 0; mu < 4; ++mu)
+        if (L[mu] < 2 || (L[mu] & 1)) return -1;
+    const long n = vol(L) / 2 * 6;
+    std::vector<std::vector<double> > w(nshift, std::vector<double>(n));
+    for (int i = 0; i < nshift; ++i)
+        if (oracle_dslash(L, links, x + (long)i * n, w[i].data(), 1)) return -1;
+    const cd *U = reinterpret_cast<const cd *>(links);
+    cd *F = reinterpret_cast<cd *>(force);
+    for (int x3 = 0; x3 < L[3]; ++x3)
+        for (int x2 = 0; x2 < L[2]; ++x2)
+            for (int x1 = 0; x1 < L[1]; ++x1)
+                for (int x0 = 0; x0 < L[0]; ++x0) {
+                    const int xx[4] = {x0, x1, x2, x3};
+                    const long lz = lex_of(L, x0, x1, x2, x3);
+                    const int par = (x0 + x1 + x2 + x3) & 1;
+                    const double eps = par ? -1.0 : 1.0;
+                    int phase_sum = 0;
+                    for (int mu = 0; mu < 4; ++mu) {
+                        const double eta = (phase_sum & 1) ? -1.0 : 1.0;
+                        const double sgn = (mu == 3 && xx[3] == L[3] - 1) ? -1.0 : 1.0;
+                        const double f = 0.5 * eta * sgn;
+                        int xp[4] = {x0, x1, x2, x3};
+                        xp[mu] = (xx[mu] + 1) % L[mu];
+                        const long lzp = lex_of(L, xp[0], xp[1], xp[2], xp[3]);
+                        cd M[9];
+                        for (int k = 0; k < 9; ++k) M[k] = 0.0;
+                        for (int i = 0; i < nshift; ++i) {
+                            const cd *xe = reinterpret_cast<const cd *>(x + (long)i * n);
+                            const cd *wo = reinterpret_cast<const cd *>(w[i].data());
+                            const cd *Xz = (par == 0 ? xe : wo) + (lz / 2) * 3;
+                            const cd *Xzp = (par == 0 ? wo : xe) + (lzp / 2) * 3;
+                            for (int a = 0; a < 3; ++a)
+                                for (int b = 0; b < 3; ++b)
+                                    M[a * 3 + b] += eps * residues[i] * Xzp[a] * std::conj(Xz[b]);
+                        }
+                        const cd *Ul = U + (lz * 4 + mu) * 9;
+                        cd G[9];
+                        for (int a = 0; a < 3; ++a)
+                            for (int b = 0; b < 3; ++b) {
+                                cd t = 0.0;
+                                for (int c = 0; c < 3; ++c) t += Ul[a * 3 + c] * M[c * 3 + b];
+                                G[a * 3 + b] = t;
+                            }
+                        cd tr = 0.0;
+                        for (int a = 0; a < 3; ++a) tr += G[a * 3 + a] - std::conj(G[a * 3 + a]);
+                        cd *Fl = F + (lz * 4 + mu) * 9;
+                        for (int a = 0; a < 3; ++a)
+                            for (int b = 0; b < 3; ++b) {
+                                cd t = 0.5 * (G[a * 3 + b] - std::conj(G[b * 3 + a]));
+                                if (a == b) t -= tr / 6.0;
+                                Fl[a * 3 + b] = 2.0 * f * t;
+                            }
+                        phase_sum += xx[mu];
+                    }
+                }
+    return 0;
 }
 
 // y = residue0*b + sum_i residues[i]*x_i   (partial-fraction form of r(A) b)

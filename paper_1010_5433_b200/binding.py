@@ -26,6 +26,7 @@ SYMBOLS = [
     "stag_dslash_block", "stag_cg_block_workspace_bytes", "stag_mshift_cg_block",
     "stag_vector_convert", "stag_cg_polish_workspace_bytes", "stag_cg_polish",
     "stag_mshift_cg_mixed_workspace_bytes", "stag_mshift_cg_mixed",
+    "stag_force_workspace_bytes", "stag_fermion_force",
 ]
 
 
@@ -114,6 +115,9 @@ def lib() -> C.CDLL:
     l.stag_mshift_cg_mixed.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
                                        C.c_double, C.c_double, C.c_double, C.c_int, _vp, _vp, _vp,
                                        C.POINTER(MixedInfo), _vp]
+    l.stag_force_workspace_bytes.argtypes = [_vp, C.c_int, C.c_int]
+    l.stag_force_workspace_bytes.restype = _sz
+    l.stag_fermion_force.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _dp, _vp, _vp, C.c_int, _vp, _vp]
     l.stag_dslash_host.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp]
     l.stag_mshift_cg_host.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
                                       C.c_double, C.c_double, C.c_int, _vp, _vp, _vp, C.POINTER(CgInfo), _vp]
@@ -306,6 +310,17 @@ class Stag:
         if check and rc not in (OK, ERR_NOTCONV, ERR_BREAKDOWN):
             raise StagError(rc, "stag_mshift_cg_mixed")
         return rc, info.as_dict(n)
+
+    # ---- N4: fermion force of the rational action
+    def force_workspace_bytes(self, prec, nshift): return lib().stag_force_workspace_bytes(self._h, prec, nshift)
+
+    def fermion_force(self, packed, prec, recon, residues, x_even, dev_force, workspace, accumulate=False,
+                      stream=None):
+        rs = _darr(residues)
+        rc = lib().stag_fermion_force(self._h, _ptr(packed), prec, recon, rs[1].size, rs[0], _ptr(x_even),
+                                      _ptr(dev_force), int(bool(accumulate)), _ptr(workspace), _stream(stream))
+        if rc:
+            raise StagError(rc, "stag_fermion_force")
 
     # ---- host-buffer variants
     def dslash_host(self, packed, prec, recon, out_parity, host_in, host_out, dev_scratch, stream=None):

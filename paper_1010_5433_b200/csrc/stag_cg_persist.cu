@@ -36,7 +36,7 @@ int cg_persistent_dispatch(const stag_ctx *ctx, const void *packed, int prec, in
     a.state_stride = align256(sizeof(CgState));
     a.partials = reinterpret_cast<double *>(ws + lay.partials);
     a.nrhs = 1;
-    if (prec == STAG_F64_SPLIT) return cg_persistent_launch_split(ctx, recon, a, st);
+    if (prec == STAG_F64_SPLIT) return cg_persistent_launch_split(ctx, recon, 1, a, st);
     return cg_persistent_launch_r<1>(ctx, prec, recon, a, st);
 }
 
@@ -148,8 +148,7 @@ int stag::block_solve(const stag_ctx *ctx, const void *packed, int prec, int rec
     a.state_stride = lay.state_stride;
     a.partials = reinterpret_cast<double *>(ws + lay.partials);
     a.nrhs = nrhs;
-    if (prec == STAG_F64_SPLIT && nrhs != 1) return STAG_ERR_UNSUPPORTED;
-    int rc = prec == STAG_F64_SPLIT ? cg_persistent_launch_split(ctx, recon, a, st)
+    int rc = prec == STAG_F64_SPLIT ? cg_persistent_launch_split(ctx, recon, nrhs == 1 ? 1 : nrhs == 2 ? 2 : 4, a, st)
            : nrhs == 1 ? cg_persistent_launch_r<1>(ctx, prec, recon, a, st)
            : nrhs == 2 ? cg_persistent_launch_r<2>(ctx, prec, recon, a, st)
                        : cg_persistent_launch_r<4>(ctx, prec, recon, a, st);

@@ -605,8 +605,8 @@ int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t
 template <int R>
 int cg_persistent_launch_r(const stag_ctx *ctx, int prec, int recon, const PersistArgs &a, cudaStream_t st);
 
-// N3: single source on split-double links (stag_cg_persist_split.cu)
-int cg_persistent_launch_split(const stag_ctx *ctx, int recon, const PersistArgs &a, cudaStream_t st);
+// N3: split-double links (stag_cg_persist_split.cu); R = 1, 2 or 4 sources compiled in
+int cg_persistent_launch_split(const stag_ctx *ctx, int recon, int R, const PersistArgs &a, cudaStream_t st);
 
 #define STAG_DEFINE_PERSIST_R(RR)                                                                       \
     template <>                                                                                         \

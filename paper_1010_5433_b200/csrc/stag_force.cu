@@ -1,0 +1,131 @@
+// stag_force.cu — N4: the first consumer of the multi-shift solutions, the fermion
+// force of the rational pseudo-fermion action (PAPER.md:25 "fermion force", :93 "the inversions needed
+// in the fermion force calculation"), one thread per link as in the paper's gauge update.
+//
+//   X_i = x_i on even sites, w_i = D_oe x_i on odd sites;  eps(z) = +1 even / -1 odd
+//   M_mu(z) = eps(z) sum_i residues_i X_i(z+mu) X_i(z)^dag
+//   F_mu(z) = 2 TA( W_mu(z) M_mu(z) ),  W_mu(z) = f U_mu(z) = the packed FORWARD hopping matrix of z
+//   TA(G) = (G - G^dag)/2 - tr(G - G^dag)/6
+// so that d/dt S[U_mu(z) -> exp(itT) U_mu(z)] = tr(i T F_mu(z))  (derivation: DESIGN.md "N4").
+// The factor f = 1/2 eta s of the hop is already folded into the packed matrix, so the kernel reads
+// exactly the buffers the solver used: no second copy of the gauge field.
+#include "stag_dslash.cuh"
+
+namespace stag {
+
+struct ForceCoef { double a[STAG_MAX_SHIFTS]; };
+
+// blockIdx.y = par * 4 + mu;  thread = one link (z, mu), z = site e of parity par
+template <typename T, int RECON>
+__global__ void __launch_bounds__(128)
+force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ x_even,
+             const char *__restrict__ w_odd, const size_t stride, const int nshift, const ForceCoef coef,
+             double *__restrict__ force, const int accumulate) {
+    const int e = blockIdx.x * 128 + threadIdx.x;
+    if (e >= g.Vh) return;
+    const int par = blockIdx.y >> 2, mu = blockIdx.y & 3;
+    const Site s = site_of(g, e, par);
+    const int Vh = g.Vh;
+    const int x[4] = {s.x0, s.x1, s.x2, s.x3};
+    int str = 1, phase_sum = 0;
+    for (int nu = 0; nu < mu; ++nu) { str *= g.L[nu]; phase_sum += x[nu]; }
+    const int Lmu = g.L[mu];
+    const int ef = (s.lex + str - (x[mu] == Lmu - 1 ? Lmu * str : 0)) >> 1;
+    T c3 = T(0);
+    if (RECON == 12) {
+        const T eta = (phase_sum & 1) ? T(-2) : T(2);
+        c3 = (mu == 3 && x[3] == Lmu - 1) ? -eta : eta;
+    }
+    const char *own = par == 0 ? x_even : w_odd;     // X_i(z)
+    const char *nbr = par == 0 ? w_odd : x_even;     // X_i(z + mu)
+    T m[18];
+#pragma unroll
+    for (int k = 0; k < 18; ++k) m[k] = T(0);
+    for (int i = 0; i < nshift; ++i) {
+        T a[6], b[6];
+        load_vec(own + (size_t)i * stride, Vh, e, a);
+        load_vec(nbr + (size_t)i * stride, Vh, ef, b);
+        const T c = (T)coef.a[i];
+#pragma unroll
+        for (int r = 0; r < 3; ++r) {
+            const T br = c * b[2 * r], bi = c * b[2 * r + 1];
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {            // M[r][q] += c b_r conj(a_q)
+                m[6 * r + 2 * q] = fma(br, a[2 * q], fma(bi, a[2 * q + 1], m[6 * r + 2 * q]));
+                m[6 * r + 2 * q + 1] = fma(bi, a[2 * q], fma(-br, a[2 * q + 1], m[6 * r + 2 * q + 1]));
+            }
+        }
+    }
+    T u[18];
+    const size_t set = link_set_bytes<T, RECON>(Vh);
+    load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3, policy_evict_first());
+    // G = W M in fp64 (one 3x3 product per link: free next to the loads)
+    double G[18];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            double re = 0.0, im = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double ur = u[6 * r + 2 * k], ui = u[6 * r + 2 * k + 1];
+                const double mr = m[6 * k + 2 * q], mi = m[6 * k + 2 * q + 1];
+                re += ur * mr - ui * mi;
+                im += ur * mi + ui * mr;
+            }
+            G[6 * r + 2 * q] = re; G[6 * r + 2 * q + 1] = im;
+        }
+    const double eps2 = par ? -2.0 : 2.0;            // 2 eps(z)
+    const double tr_im = (G[1] + G[9] + G[17]) * (2.0 / 6.0);     // tr(G - G^dag)/6 = i * 2 Im tr G / 6
+    double *out = force + ((size_t)s.lex * 4 + mu) * 18;
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            double re = 0.5 * (G[6 * r + 2 * q] - G[6 * q + 2 * r]);
+            double im = 0.5 * (G[6 * r + 2 * q + 1] + G[6 * q + 2 * r + 1]);
+            if (r == q) im -= tr_im;
+            re *= eps2; im *= eps2;
+            if (accumulate) { re += out[6 * r + 2 * q]; im += out[6 * r + 2 * q + 1]; }
+            out[6 * r + 2 * q] = re; out[6 * r + 2 * q + 1] = im;
+        }
+}
+
+}  // namespace stag
+
+using namespace stag;
+
+extern "C" size_t stag_force_workspace_bytes(const stag_ctx *ctx, int prec, int nshift) {
+    if (!ctx || (prec != STAG_F64 && prec != STAG_F32) || nshift < 1 || nshift > STAG_MAX_SHIFTS) return 0;
+    return align256((size_t)nshift * ctx->g.Vh * vec_bytes_per_site(prec));
+}
+
+extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int prec, int recon, int nshift,
+                                  const double *host_residues, const void *x_even, double *dev_force,
+                                  int accumulate, void *workspace, void *stream) {
+    if (!ctx || !packed || !host_residues || !x_even || !dev_force || !workspace) return STAG_ERR_BADARG;
+    if ((prec != STAG_F64 && prec != STAG_F32) || !valid_recon(recon)) return prec == STAG_F64_SPLIT ? STAG_ERR_UNSUPPORTED : STAG_ERR_BADARG;
+    if (nshift < 1 || nshift > STAG_MAX_SHIFTS) return STAG_ERR_BADARG;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const Geom &g = ctx->g;
+    const size_t vbytes = (size_t)g.Vh * vec_bytes_per_site(prec);
+    const char *x = static_cast<const char *>(x_even);
+    char *w = static_cast<char *>(workspace);
+    // w_i = D_oe x_i, STAG_MAX_RHS shifts per read of the links (N1 kernel)
+    for (int i0 = 0; i0 < nshift; i0 += STAG_MAX_RHS) {
+        const int n = nshift - i0 < STAG_MAX_RHS ? nshift - i0 : STAG_MAX_RHS;
+        const int rc = stag_dslash_block(ctx, packed, prec, recon, 1, n, x + (size_t)i0 * vbytes,
+                                         w + (size_t)i0 * vbytes, st);
+        if (rc) return rc;
+    }
+    ForceCoef coef;
+    for (int i = 0; i < STAG_MAX_SHIFTS; ++i) coef.a[i] = i < nshift ? host_residues[i] : 0.0;
+    const dim3 grid((g.Vh + 127) / 128, 8), block(128);
+    const char *W = static_cast<const char *>(packed);
+#define STAG_FORCE(T, R) force_kernel<T, R><<<grid, block, 0, st>>>(g, W, x, w, vbytes, nshift, coef, dev_force, accumulate)
+    if (prec == STAG_F64) { if (recon == 18) STAG_FORCE(double, 18); else STAG_FORCE(double, 12); }
+    else { if (recon == 18) STAG_FORCE(float, 18); else STAG_FORCE(float, 12); }
+#undef STAG_FORCE
+    STAG_CUDA_OK(cudaGetLastError());
+    return STAG_OK;
+}

@@ -119,7 +119,7 @@ static int polish(const stag_ctx *ctx, const void *packed, int prec, int recon, 
     unsigned int *ticket = reinterpret_cast<unsigned int *>(ws + lay.scal + 128);
     double *partials = reinterpret_cast<double *>(ws + lay.partials);
     volatile double *hn = reinterpret_cast<volatile double *>(reinterpret_cast<char *>(ctx->pinned_flags) + 128);
-    const int group = prec == STAG_F64 ? STAG_MAX_RHS : 1;
+    const int group = STAG_MAX_RHS;    // the defects of a split-double group are one Dslash launch per shift (dslash_n)
     stag_polish_info pi;
     std::memset(&pi, 0, sizeof(pi));
     int launches = 0;

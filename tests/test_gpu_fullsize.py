@@ -94,6 +94,27 @@ def test_c4_dslash_block_four_sources(stag, c4, prec, recon, pipe):
         assert rel(ctx.download_vector(vout, prec, k * vb), oracle.dslash_oe(L, U, srcs[k])) <= TOL[prec]
 
 
+def test_c4_mixed_precision_on_one_split_buffer(stag, c4):
+    """N2 + N3 at full size, as bench.py times it: fp32 multi-shift on the b planes, fp64 polish on b + c of
+    the SAME buffer; true residual of every shift by the oracle's operator on the unsplit links."""
+    cfg, U, srcs = c4
+    L, m, shifts, stop = cfg["L"], cfg["mass"], cfg["shifts"], cfg["stops"][0]
+    ctx = stag.Stag(L)
+    split = ctx.upload_gauge(U, stag.F64_SPLIT, 18)
+    n, vb = len(shifts), ctx.vector_bytes(stag.F64)
+    x, ws = ctx.alloc(n * vb), ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(n))
+    b = srcs[2]
+    rc, info = ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, ctx.upload_vector(b, stag.F64), m, shifts,
+                                   stop, 100000, x, ws)
+    assert rc == 0, info
+    nb = np.linalg.norm(b)
+    for i, s in enumerate(shifts):
+        xi = ctx.download_vector(x, stag.F64, i * vb)
+        tr = np.linalg.norm(b - oracle.apply_A(L, U, m, s, xi)) / nb
+        assert tr <= stop, (i, tr)
+        assert abs(tr - info["polish"]["resid_after"][i]) <= 0.1 * stop
+
+
 def test_c4_block_cg_four_sources(stag, c4):
     """The block solve bench.py reports: 4 sources x 16 shifts in one persistent launch; true residual of
     every (source, shift) by the oracle's operator, iteration counts equal to the single-source path's."""

@@ -384,3 +384,76 @@ def test_P9_polish_of_the_exact_solution_and_bad_args():
     assert oracle.cg_polish(L, U, b, m, 0.3, np.zeros_like(b), 1e-30, 3)["rc"] == -5
     with pytest.raises(ValueError):
         oracle.cg_polish(L, U, b, m, 0.3, xd, 0.0, 10)
+
+
+# ---- N4: fermion force = derivative of the rational pseudo-fermion action ---------
+GELL_MANN = np.zeros((8, 3, 3), dtype=np.complex128)
+GELL_MANN[0][0, 1] = GELL_MANN[0][1, 0] = 1
+GELL_MANN[1][0, 1], GELL_MANN[1][1, 0] = -1j, 1j
+GELL_MANN[2][0, 0], GELL_MANN[2][1, 1] = 1, -1
+GELL_MANN[3][0, 2] = GELL_MANN[3][2, 0] = 1
+GELL_MANN[4][0, 2], GELL_MANN[4][2, 0] = -1j, 1j
+GELL_MANN[5][1, 2] = GELL_MANN[5][2, 1] = 1
+GELL_MANN[6][1, 2], GELL_MANN[6][2, 1] = -1j, 1j
+GELL_MANN[7][0, 0] = GELL_MANN[7][1, 1] = 1 / np.sqrt(3)
+GELL_MANN[7][2, 2] = -2 / np.sqrt(3)
+
+
+def _expi(T, t):
+    w, v = np.linalg.eigh(T)
+    return (v * np.exp(1j * t * w)) @ v.conj().T
+
+
+def _action(L, U, b, m, shifts, residues, residue0):
+    """S = b^dag (residue0 + sum_i residues_i (A + sigma_i)^-1) b from DENSE solves (oracle_dense_*, pinned by P7)."""
+    A = oracle.dense_A(L, U, m)
+    bv = b.reshape(-1)
+    S = residue0 * np.vdot(bv, bv).real
+    for s, a in zip(shifts, residues):
+        S += a * np.vdot(bv, oracle.dense_solve(A, s, b)).real
+    return S
+
+
+@pytest.mark.parametrize("L,links", [((2, 2, 2, 2), [(0, 0), (3, 3), (9, 3), (12, 1), (15, 2)]),
+                                     ((4, 4, 2, 2), [(0, 0), (5, 1), (13, 2), (35, 3), (62, 3), (63, 0)])])
+def test_P10_force_is_the_derivative_of_the_action(L, links):
+    """d/dt S[U_mu(z) -> exp(itT) U_mu(z)] = tr(i T F_mu(z)), central differences, all 8 generators, links on
+    both parities, in every direction and on the antiperiodic layer (x3 = L3 - 1: sites 9.. of 2^4 / 35, 62 of 4.4.2.2)."""
+    U, b, m = si.links_haar(L, 61), si.source_gaussian(L, 61), 0.3
+    shifts, residues, residue0 = [0.05, 0.4, 1.7], [0.7, -0.3, 1.9], 0.4
+    A = oracle.dense_A(L, U, m)
+    x = np.stack([oracle.dense_solve(A, s, b).reshape(-1, 3) for s in shifts])
+    F = oracle.fermion_force(L, U, residues, x)
+    eps = 1e-4
+    for z, mu in links:
+        for T in GELL_MANN:
+            Up, Um = U.copy(), U.copy()
+            Up[z, mu] = _expi(T, eps) @ U[z, mu]
+            Um[z, mu] = _expi(T, -eps) @ U[z, mu]
+            fd = (_action(L, Up, b, m, shifts, residues, residue0) - _action(L, Um, b, m, shifts, residues, residue0)) / (2 * eps)
+            an = np.trace(1j * T @ F[z, mu])
+            assert abs(an.imag) <= 1e-12 * max(1.0, abs(an.real))
+            assert abs(fd - an.real) <= 2e-6 * max(1.0, np.abs(F[z, mu]).max()), (z, mu, fd, an)
+
+
+def test_P10_force_is_traceless_antihermitian_and_gauge_covariant():
+    L = (4, 4, 4, 4)
+    U, m = si.links_haar(L, 62), 0.1
+    residues = [1.0, 0.5]
+    rng = np.random.default_rng(3)
+    x = rng.standard_normal((2, 128, 3)) + 1j * rng.standard_normal((2, 128, 3))   # any even-site vectors do
+    F = oracle.fermion_force(L, U, residues, x)
+    assert np.abs(F + F.conj().transpose(0, 1, 3, 2)).max() <= 1e-14 * np.abs(F).max()
+    assert np.abs(np.trace(F, axis1=2, axis2=3)).max() <= 1e-14 * np.abs(F).max()
+    assert np.abs(F).max() > 0.1
+    # U' = g U g^dag(x+mu), x' = g x  =>  F'_mu(z) = g(z) F_mu(z) g(z)^dag
+    g = si.gauge_transform_field(L, 62)
+    Ug = si.apply_gauge_transform(L, U, g)
+    ge = g[si.parity_sites(L, 0)]
+    xg = np.einsum("sab,isb->isa", ge, x)
+    Fg = oracle.fermion_force(L, Ug, residues, xg)
+    want = np.einsum("zab,zmbc,zdc->zmad", g, F, g.conj())
+    assert rel(Fg, want) <= 1e-13
+    # linear in the residues, quadratic in x
+    assert rel(oracle.fermion_force(L, U, [2.0, 1.0], x), 2 * F) <= 1e-14
+    assert rel(oracle.fermion_force(L, U, residues, 3 * x), 9 * F) <= 1e-14
