@@ -312,6 +312,35 @@ def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
     return out
 
 
+def measure_force(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh):
+    """N4: stag_fermion_force on nshift even vectors (the x_i of a solve; timing does not depend on their
+    values, so the sources stand in), 20 calls between CUDA events after 3 warm-up calls.  Algorithmic bytes:
+    D_oe x_i through the multi-source kernel (links once per group of 4, each vector read + written once) +
+    per link one matrix, one 144-byte output, and every X_i read once."""
+    n = len(cfg["shifts"])
+    w = 4 if prec == stag.F32 else 8
+    x = ctx.upload_vectors([srcs[k % len(srcs)] for k in range(n)], prec)
+    F = torch.empty(2 * vh * 72, dtype=torch.float64, device="cuda")
+    ws = ctx.alloc(ctx.force_workspace_bytes(prec, n))
+    res = [1.0 / (i + 1) for i in range(n)]
+    for _ in range(3):
+        ctx.fermion_force(packed, prec, recon, res, x, F, ws)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(20):
+        ctx.fermion_force(packed, prec, recon, res, x, F, ws)
+    e1.record()
+    torch.cuda.synchronize()
+    secs = e0.elapsed_time(e1) * 1e-3 / 20
+    groups = (n + 3) // 4
+    bytes_dslash = vh * (groups * 8 * recon * w + n * 2 * 6 * w)
+    bytes_force = 2 * vh * (4 * recon * w + 4 * 144 + n * 6 * w)
+    gbs = (bytes_dslash + bytes_force) / secs / 1e9
+    return {"us_per_call": secs * 1e6, "nshift": n, "launches_per_call": 1 + groups,
+            "algorithmic_bytes_per_call": bytes_dslash + bytes_force, "gbs_algorithmic": gbs}
+
+
 def dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, pack_ms, gen_s):
     """--dslash-only: the SURVEY.md §8(d) Dslash bandwidth sweep alone (no CG), one JSON line."""
     peak, peak_src = measured_peak_gbs()
@@ -485,6 +514,11 @@ def run_ours(args):
     if rank == 0 and not args.no_block and prec == stag.F64:
         mixed = measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, secs / args.steps)
 
+    force = None
+    if rank == 0 and not args.no_block and prec != stag.F64_SPLIT:
+        force = measure_force(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh)
+        force["pct_of_measured"] = 100 * force["gbs_algorithmic"] / peak
+
     # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -506,7 +540,7 @@ def run_ours(args):
                       "gbs_algorithmic": cg_gbs, "pct_of_8tbs": 100 * cg_gbs / NOMINAL_HBM_GBS,
                       "pct_of_measured": 100 * cg_gbs / peak, "solves": nsolves,
                       "iters_shift_first_solve": infos[0]["iters_shift"]},
-               "dslash": dslash, "block": block, "mixed": mixed, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
+               "dslash": dslash, "block": block, "mixed": mixed, "force": force, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
                "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
                        "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": te_s / e2e_steps,
                        "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},

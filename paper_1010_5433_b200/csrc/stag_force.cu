@@ -15,80 +15,96 @@ namespace stag {
 
 struct ForceCoef { double a[STAG_MAX_SHIFTS]; };
 
-// blockIdx.y = par * 4 + mu;  thread = one link (z, mu), z = site e of parity par
+// CTA = 32 consecutive sites of one parity (blockIdx.y) x 4 directions; thread = one link (z, mu), mu the
+// fastest thread index: the 4 threads of a site share every load of X_i(z) (one broadcast request), and the
+// CTA's 128 matrices (32 runs of 576 contiguous bytes in the canonical layout) leave through shared memory
+// as full 32-byte sectors instead of 16-byte pieces scattered over 128 lines per store instruction.
 template <typename T, int RECON>
 __global__ void __launch_bounds__(128)
 force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ x_even,
              const char *__restrict__ w_odd, const size_t stride, const int nshift, const ForceCoef coef,
              double *__restrict__ force, const int accumulate) {
-    const int e = blockIdx.x * 128 + threadIdx.x;
-    if (e >= g.Vh) return;
-    const int par = blockIdx.y >> 2, mu = blockIdx.y & 3;
-    const Site s = site_of(g, e, par);
+    __shared__ double2 stage[128 * 9];                 // [site][mu][9 complex]
+    __shared__ int s_lex[32];
+    const int mu = threadIdx.x & 3, ls = threadIdx.x >> 2, par = blockIdx.y, tile = blockIdx.x;
+    const int e = tile * 32 + ls;
     const int Vh = g.Vh;
-    const int x[4] = {s.x0, s.x1, s.x2, s.x3};
-    int str = 1, phase_sum = 0;
-    for (int nu = 0; nu < mu; ++nu) { str *= g.L[nu]; phase_sum += x[nu]; }
-    const int Lmu = g.L[mu];
-    const int ef = (s.lex + str - (x[mu] == Lmu - 1 ? Lmu * str : 0)) >> 1;
-    T c3 = T(0);
-    if (RECON == 12) {
-        const T eta = (phase_sum & 1) ? T(-2) : T(2);
-        c3 = (mu == 3 && x[3] == Lmu - 1) ? -eta : eta;
-    }
-    const char *own = par == 0 ? x_even : w_odd;     // X_i(z)
-    const char *nbr = par == 0 ? w_odd : x_even;     // X_i(z + mu)
-    T m[18];
+    const bool on = e < Vh;
+    if (on) {
+        const Site s = site_of(g, e, par);
+        if (mu == 0) s_lex[ls] = s.lex;
+        const int x[4] = {s.x0, s.x1, s.x2, s.x3};
+        int str = 1, phase_sum = 0;
+        for (int nu = 0; nu < mu; ++nu) { str *= g.L[nu]; phase_sum += x[nu]; }
+        const int Lmu = g.L[mu];
+        const int ef = (s.lex + str - (x[mu] == Lmu - 1 ? Lmu * str : 0)) >> 1;
+        T c3 = T(0);
+        if (RECON == 12) {
+            const T eta = (phase_sum & 1) ? T(-2) : T(2);
+            c3 = (mu == 3 && x[3] == Lmu - 1) ? -eta : eta;
+        }
+        T u[18];
+        const size_t set = link_set_bytes<T, RECON>(Vh);
+        load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3, policy_evict_first());
+        const char *own = par == 0 ? x_even : w_odd;     // X_i(z)
+        const char *nbr = par == 0 ? w_odd : x_even;     // X_i(z + mu)
+        T m[18];
 #pragma unroll
-    for (int k = 0; k < 18; ++k) m[k] = T(0);
-    for (int i = 0; i < nshift; ++i) {
-        T a[6], b[6];
-        load_vec(own + (size_t)i * stride, Vh, e, a);
-        load_vec(nbr + (size_t)i * stride, Vh, ef, b);
-        const T c = (T)coef.a[i];
+        for (int k = 0; k < 18; ++k) m[k] = T(0);
+#pragma unroll 4
+        for (int i = 0; i < nshift; ++i) {
+            T a[6], b[6];
+            load_vec(own + (size_t)i * stride, Vh, e, a);
+            load_vec(nbr + (size_t)i * stride, Vh, ef, b);
+            const T c = (T)coef.a[i];
 #pragma unroll
-        for (int r = 0; r < 3; ++r) {
-            const T br = c * b[2 * r], bi = c * b[2 * r + 1];
+            for (int r = 0; r < 3; ++r) {
+                const T br = c * b[2 * r], bi = c * b[2 * r + 1];
 #pragma unroll
-            for (int q = 0; q < 3; ++q) {            // M[r][q] += c b_r conj(a_q)
-                m[6 * r + 2 * q] = fma(br, a[2 * q], fma(bi, a[2 * q + 1], m[6 * r + 2 * q]));
-                m[6 * r + 2 * q + 1] = fma(bi, a[2 * q], fma(-br, a[2 * q + 1], m[6 * r + 2 * q + 1]));
+                for (int q = 0; q < 3; ++q) {            // M[r][q] += c b_r conj(a_q)
+                    m[6 * r + 2 * q] = fma(br, a[2 * q], fma(bi, a[2 * q + 1], m[6 * r + 2 * q]));
+                    m[6 * r + 2 * q + 1] = fma(bi, a[2 * q], fma(-br, a[2 * q + 1], m[6 * r + 2 * q + 1]));
+                }
             }
         }
-    }
-    T u[18];
-    const size_t set = link_set_bytes<T, RECON>(Vh);
-    load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3, policy_evict_first());
-    // G = W M in fp64 (one 3x3 product per link: free next to the loads)
-    double G[18];
+        // G = W M in fp64 (one 3x3 product per link: free next to the loads)
+        double G[18];
 #pragma unroll
-    for (int r = 0; r < 3; ++r)
+        for (int r = 0; r < 3; ++r)
 #pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            double re = 0.0, im = 0.0;
+            for (int q = 0; q < 3; ++q) {
+                double re = 0.0, im = 0.0;
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const double ur = u[6 * r + 2 * k], ui = u[6 * r + 2 * k + 1];
-                const double mr = m[6 * k + 2 * q], mi = m[6 * k + 2 * q + 1];
-                re += ur * mr - ui * mi;
-                im += ur * mi + ui * mr;
+                for (int k = 0; k < 3; ++k) {
+                    const double ur = u[6 * r + 2 * k], ui = u[6 * r + 2 * k + 1];
+                    const double mr = m[6 * k + 2 * q], mi = m[6 * k + 2 * q + 1];
+                    re += ur * mr - ui * mi;
+                    im += ur * mi + ui * mr;
+                }
+                G[6 * r + 2 * q] = re; G[6 * r + 2 * q + 1] = im;
             }
-            G[6 * r + 2 * q] = re; G[6 * r + 2 * q + 1] = im;
-        }
-    const double eps2 = par ? -2.0 : 2.0;            // 2 eps(z)
-    const double tr_im = (G[1] + G[9] + G[17]) * (2.0 / 6.0);     // tr(G - G^dag)/6 = i * 2 Im tr G / 6
-    double *out = force + ((size_t)s.lex * 4 + mu) * 18;
+        const double eps2 = par ? -2.0 : 2.0;            // 2 eps(z)
+        const double tr_im = (G[1] + G[9] + G[17]) * (2.0 / 6.0);     // tr(G - G^dag)/6 = i * 2 Im tr G / 6
 #pragma unroll
-    for (int r = 0; r < 3; ++r)
+        for (int r = 0; r < 3; ++r)
 #pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            double re = 0.5 * (G[6 * r + 2 * q] - G[6 * q + 2 * r]);
-            double im = 0.5 * (G[6 * r + 2 * q + 1] + G[6 * q + 2 * r + 1]);
-            if (r == q) im -= tr_im;
-            re *= eps2; im *= eps2;
-            if (accumulate) { re += out[6 * r + 2 * q]; im += out[6 * r + 2 * q + 1]; }
-            out[6 * r + 2 * q] = re; out[6 * r + 2 * q + 1] = im;
-        }
+            for (int q = 0; q < 3; ++q) {
+                double re = 0.5 * (G[6 * r + 2 * q] - G[6 * q + 2 * r]);
+                double im = 0.5 * (G[6 * r + 2 * q + 1] + G[6 * q + 2 * r + 1]);
+                if (r == q) im -= tr_im;
+                stage[threadIdx.x * 9 + 3 * r + q] = make_double2(re * eps2, im * eps2);
+            }
+    }
+    __syncthreads();
+    // 32 sites x 36 chunks of 16 bytes; consecutive threads write consecutive chunks of one site
+    const int nsite = min(32, Vh - tile * 32);
+    for (int k = threadIdx.x; k < nsite * 36; k += 128) {
+        const int site = k / 36, c = k - site * 36;
+        double2 v = stage[site * 36 + c];
+        double2 *out = reinterpret_cast<double2 *>(force + (size_t)s_lex[site] * 72) + c;
+        if (accumulate) { const double2 o = *out; v.x += o.x; v.y += o.y; }
+        *out = v;
+    }
 }
 
 }  // namespace stag
@@ -120,7 +136,7 @@ extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int p
     }
     ForceCoef coef;
     for (int i = 0; i < STAG_MAX_SHIFTS; ++i) coef.a[i] = i < nshift ? host_residues[i] : 0.0;
-    const dim3 grid((g.Vh + 127) / 128, 8), block(128);
+    const dim3 grid((g.Vh + 31) / 32, 2), block(128);
     const char *W = static_cast<const char *>(packed);
 #define STAG_FORCE(T, R) force_kernel<T, R><<<grid, block, 0, st>>>(g, W, x, w, vbytes, nshift, coef, dev_force, accumulate)
     if (prec == STAG_F64) { if (recon == 18) STAG_FORCE(double, 18); else STAG_FORCE(double, 12); }

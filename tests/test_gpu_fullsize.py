@@ -115,6 +115,22 @@ def test_c4_mixed_precision_on_one_split_buffer(stag, c4):
         assert abs(tr - info["polish"]["resid_after"][i]) <= 0.1 * stop
 
 
+@pytest.mark.parametrize("prec", [0, 1])
+def test_c4_fermion_force(stag, c4, prec):
+    """N4 at full size, as bench.py times it: 16 vectors, every link of the 32^3 x 8 lattice against the oracle."""
+    import torch
+    cfg, U, srcs = c4
+    L, n = cfg["L"], len(cfg["shifts"])
+    xs = [srcs[k % 4] * (1.0 + 0.1 * k) for k in range(n)]
+    res = [1.0 / (i + 1) for i in range(n)]
+    ctx = stag.Stag(L)
+    packed = ctx.upload_gauge(U, prec, 18)
+    F = torch.empty(ctx.V * 72, dtype=torch.float64, device="cuda")
+    ctx.fermion_force(packed, prec, 18, res, ctx.upload_vectors(xs, prec), F, ctx.alloc(ctx.force_workspace_bytes(prec, n)))
+    got = F.cpu().numpy().view(np.complex128).reshape(ctx.V, 4, 3, 3)
+    assert rel(got, oracle.fermion_force(L, U, res, np.stack(xs))) <= TOL[prec]
+
+
 def test_c4_block_cg_four_sources(stag, c4):
     """The block solve bench.py reports: 4 sources x 16 shifts in one persistent launch; true residual of
     every (source, shift) by the oracle's operator, iteration counts equal to the single-source path's."""
