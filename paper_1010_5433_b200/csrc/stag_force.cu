@@ -15,22 +15,28 @@ namespace stag {
 
 struct ForceCoef { double a[STAG_MAX_SHIFTS]; };
 
-// CTA = 32 consecutive sites of one parity (blockIdx.y) x 4 directions; thread = one link (z, mu), mu the
-// fastest thread index: the 4 threads of a site share every load of X_i(z) (one broadcast request), and the
-// CTA's 128 matrices (32 runs of 576 contiguous bytes in the canonical layout) leave through shared memory
-// as full 32-byte sectors instead of 16-byte pieces scattered over 128 lines per store instruction.
+// CTA = 32 consecutive sites of parity blockIdx.y x 4 directions; thread = one link (z, mu) with mu = the
+// WARP index, so every 128-bit load instruction of a warp covers 32 consecutive sites (one 128-byte line per
+// quarter-warp).  Two earlier mappings, both measured (profiles/README.md, N4): mu as the fastest LANE index
+// made each gather of X_i(z+mu) touch 4 lines per quarter-warp and the kernel sat at 74 % of
+// l1tex__data_pipe_lsu_wavefronts; one thread per site with all 4 directions needs 144 fp64 accumulators,
+// leaves 8 warps per SM and is latency-bound (12 % warps active).  Here a thread keeps one 3x3 sum (36
+// registers), which leaves room to unroll the shift loop by 4: 24 independent 16-byte loads in flight per
+// thread at 12+ warps per SM.  X_i(z) is requested by the 4 warps of a CTA (3 of the 4 hit L1).
+// The CTA's 32 x 576 contiguous output bytes leave through shared memory as full sectors.
+constexpr int kForceRow = 37;                          // 36 chunks of 16 B per site + 1 pad: conflict-free
+
 template <typename T, int RECON>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, 3)
 force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ x_even,
              const char *__restrict__ w_odd, const size_t stride, const int nshift, const ForceCoef coef,
              double *__restrict__ force, const int accumulate) {
-    __shared__ double2 stage[128 * 9];                 // [site][mu][9 complex]
+    __shared__ double2 stage[32 * kForceRow];          // [site][mu][9 complex] (+ pad)
     __shared__ int s_lex[32];
-    const int mu = threadIdx.x & 3, ls = threadIdx.x >> 2, par = blockIdx.y, tile = blockIdx.x;
-    const int e = tile * 32 + ls;
+    const int mu = threadIdx.x >> 5, ls = threadIdx.x & 31, par = blockIdx.y;
+    const int e = blockIdx.x * 32 + ls;
     const int Vh = g.Vh;
-    const bool on = e < Vh;
-    if (on) {
+    if (e < Vh) {
         const Site s = site_of(g, e, par);
         if (mu == 0) s_lex[ls] = s.lex;
         const int x[4] = {s.x0, s.x1, s.x2, s.x3};
@@ -43,11 +49,8 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
             const T eta = (phase_sum & 1) ? T(-2) : T(2);
             c3 = (mu == 3 && x[3] == Lmu - 1) ? -eta : eta;
         }
-        T u[18];
-        const size_t set = link_set_bytes<T, RECON>(Vh);
-        load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3, policy_evict_first());
-        const char *own = par == 0 ? x_even : w_odd;     // X_i(z)
-        const char *nbr = par == 0 ? w_odd : x_even;     // X_i(z + mu)
+        const char *own = (par == 0 ? x_even : w_odd);     // X_i(z)
+        const char *nbr = (par == 0 ? w_odd : x_even);     // X_i(z + mu)
         T m[18];
 #pragma unroll
         for (int k = 0; k < 18; ++k) m[k] = T(0);
@@ -67,6 +70,9 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
                 }
             }
         }
+        T u[18];
+        const size_t set = link_set_bytes<T, RECON>(Vh);
+        load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3, policy_evict_first());
         // G = W M in fp64 (one 3x3 product per link: free next to the loads)
         double G[18];
 #pragma unroll
@@ -85,6 +91,7 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
             }
         const double eps2 = par ? -2.0 : 2.0;            // 2 eps(z)
         const double tr_im = (G[1] + G[9] + G[17]) * (2.0 / 6.0);     // tr(G - G^dag)/6 = i * 2 Im tr G / 6
+        double2 *row = stage + ls * kForceRow + mu * 9;
 #pragma unroll
         for (int r = 0; r < 3; ++r)
 #pragma unroll
@@ -92,15 +99,15 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
                 double re = 0.5 * (G[6 * r + 2 * q] - G[6 * q + 2 * r]);
                 double im = 0.5 * (G[6 * r + 2 * q + 1] + G[6 * q + 2 * r + 1]);
                 if (r == q) im -= tr_im;
-                stage[threadIdx.x * 9 + 3 * r + q] = make_double2(re * eps2, im * eps2);
+                row[3 * r + q] = make_double2(re * eps2, im * eps2);
             }
     }
     __syncthreads();
     // 32 sites x 36 chunks of 16 bytes; consecutive threads write consecutive chunks of one site
-    const int nsite = min(32, Vh - tile * 32);
+    const int nsite = min(32, Vh - (int)blockIdx.x * 32);
     for (int k = threadIdx.x; k < nsite * 36; k += 128) {
         const int site = k / 36, c = k - site * 36;
-        double2 v = stage[site * 36 + c];
+        double2 v = stage[site * kForceRow + c];
         double2 *out = reinterpret_cast<double2 *>(force + (size_t)s_lex[site] * 72) + c;
         if (accumulate) { const double2 o = *out; v.x += o.x; v.y += o.y; }
         *out = v;
