@@ -27,7 +27,12 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-WORKLOADS = {"c2": "c2_16x16x16x4", "c3": "c3_24x24x24x6", "c4": "c4_32x32x32x8", "c5": "c5_64x64x64x64"}
+WORKLOADS = {"c2": "c2_16x16x16x4", "c3": "c3_24x24x24x6", "c4": "c4_32x32x32x8", "c5": "c5_64x64x64x64",
+             "t2b": "t2_32x32x32x32", "t2c": "t2_48x48x48x4"}
+# the paper's own Dslash figures (Table 2: Tesla C1060, fp32, 12-real, 576 flop/site by its
+# own accounting — BASELINE.md §1): context beside the fp32-12 line of the sweep, another machine's numbers
+PAPER_TABLE2 = {"c2": (49.31, 56.84, "PAPER.md:103 (4x16^3)"), "t2b": (55.597, 64.091, "PAPER.md:104 (32x32^3)"),
+                "t2c": (60.67, 69.94, "PAPER.md:105 (4x48^3)")}
 FLOP_PER_SITE = 570                                   # BASELINE.json:north_star
 DSLASH_BYTES = {(0, 18): 1248, (0, 12): 864, (1, 18): 624, (1, 12): 432,
                 (2, 18): 1248, (2, 12): 864}                               # N3 split-double: 2 floats per real
@@ -208,24 +213,43 @@ def reduce_over_ranks(torch, dist, world: int, secs: float, work, device):
 # ---------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------
-def time_dslash(torch, ctx, packed, prec, recon, a, b, launches=100, repeats=5, warm=10):
-    """SURVEY.md §8(d) protocol: warm-up launches, then CUDA events around `launches` back-to-back
-    launches ping-ponging D_oe / D_eo (outputs consumed), median of `repeats`.  Returns s per launch."""
-    def pair(n):
-        for _ in range(n // 2):
-            ctx.dslash_oe(packed, prec, recon, a, b)
-            ctx.dslash_eo(packed, prec, recon, b, a)
-    pair(warm)
+def time_launches(torch, body, launches, repeats=5):
+    """CUDA events around `launches` back-to-back launches issued by body(launches), median of `repeats`.  The
+    launches are captured once in a CUDA graph and replayed, so that on small lattices (one launch is ~8 us of
+    Python + ctypes, a 16^3x4 Dslash ~3 us) the events time the device, not the host.  Returns s per launch."""
+    run = lambda: body(launches)
+    try:
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            body(launches)
+        torch.cuda.synchronize()
+        run = graph.replay
+        run()
+    except Exception:
+        torch.cuda.synchronize()
     ts = []
     for _ in range(repeats):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         e0.record()
-        pair(launches)
+        run()
         e1.record()
         torch.cuda.synchronize()
         ts.append(e0.elapsed_time(e1) * 1e-3 / launches)
     return statistics.median(ts)
+
+
+def time_dslash(torch, ctx, packed, prec, recon, a, b, launches=100, repeats=5, warm=10):
+    """SURVEY.md §8(d) protocol: warm-up launches, then `launches` back-to-back launches ping-ponging
+    D_oe / D_eo (outputs consumed), median of `repeats`.  Returns s per launch."""
+    def pair(n):
+        for _ in range(n // 2):
+            ctx.dslash_oe(packed, prec, recon, a, b)
+            ctx.dslash_eo(packed, prec, recon, b, a)
+    pair(warm)
+    return time_launches(torch, pair, launches, repeats)
 
 
 def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
@@ -245,16 +269,7 @@ def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
                 ctx.dslash_block(packed, prec, recon, 1, R, a, b)
                 ctx.dslash_block(packed, prec, recon, 0, R, b, a)
         pair(10)
-        ts = []
-        for _ in range(5):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            e0.record()
-            pair(100)
-            e1.record()
-            torch.cuda.synchronize()
-            ts.append(e0.elapsed_time(e1) * 1e-3 / 100)
-        s_per = statistics.median(ts)
+        s_per = time_launches(torch, pair, 100)
         bps = 8 * recon * w + 2 * 6 * w * R
         gbs = bps * vh / s_per / 1e9
         out["dslash"]["R%d" % R] = {"us": s_per * 1e6, "us_per_source": s_per * 1e6 / R,
@@ -361,6 +376,13 @@ def dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, 
             "us": s_per * 1e6, "gflops": FLOP_PER_SITE * vh / s_per / 1e9, "gbs_algorithmic": gbs,
             "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak}
         del pk, a, b
+    if args.workload in PAPER_TABLE2:
+        pg, pb, cite = PAPER_TABLE2[args.workload]
+        ours = out["dslash"]["f32-12"]
+        out["paper_table2"] = {"hardware": "Tesla C1060", "prec": "f32", "recon": 12, "gflops": pg, "gbs": pb,
+                               "cite": cite, "ours_f32_12_gflops": ours["gflops"],
+                               "ratio_gflops": ours["gflops"] / pg,
+                               "note": "another machine's figure: context, not the target"}
     print(json.dumps(out))
     return 0
 

@@ -9,10 +9,13 @@ namespace stag {
 
 STAG_DEFINE_PERSIST_R(1)
 
-// single source: the persistent kernel is used when r, q and p_base all fit in shared memory
+// single source: the persistent kernel is used when at least r and q fit in shared memory (all three of
+// r, q, p_base up to Vh ~ 210 K fp64 sites; r and q up to ~ 315 K, e.g. the paper's 4 x 48^3).  Beyond that an
+// iteration takes milliseconds, launch ramps and reduction tails no longer matter, and the multi-kernel path
+// (which runs at the copy bandwidth at 64^4) is used.
 bool cg_persistent_fits(const stag_ctx *ctx, int prec) {
     const int S = sites_per_cta(ctx->g.Vh, ctx->num_sms);
-    return (size_t)3 * S * vec_bytes_per_site(prec) <= kMaxDynSmem;
+    return (size_t)2 * S * vec_bytes_per_site(prec) <= kMaxDynSmem;
 }
 
 int cg_persistent_dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon,

@@ -39,6 +39,14 @@ CONFIGS = {
         L=(64, 64, 64, 64), links=("haar", None), seed=1005, mass=0.01,
         shifts=_logspace(1e-4, 1.0, 8), residues=None, residue0=0.0,
         stops=[1e-9], nsrc=1),
+    # the two other lattices of the paper's Table 2 (4 x 16^3 is config 2's shape): Dslash
+    # timing beside the paper's C1060 figures, and a CG at the paper's N_t = 4 shape.  Seeds 1006, 1007.
+    "t2_32x32x32x32": dict(
+        L=(32, 32, 32, 32), links=("haar", None), seed=1006, mass=0.01,
+        shifts=_logspace(1e-4, 1.0, 8), residues=None, residue0=0.0, stops=[1e-9], nsrc=1),
+    "t2_48x48x48x4": dict(
+        L=(48, 48, 48, 4), links=("haar", None), seed=1007, mass=0.01,
+        shifts=_logspace(1e-4, 1.0, 8), residues=None, residue0=0.0, stops=[1e-10], nsrc=1),
 }
 
 

@@ -235,3 +235,25 @@ def test_config3_multishift_fp64(stag, stop):
     bound = stop if stop >= 1e-10 else max(stop, 1.5 * max(tr_ref))
     assert max(tr) <= bound and max(tr) <= 3 * stop, (max(tr), max(tr_ref))
     assert rel(y, oracle.partial_fraction(b, cfg["residues"], cfg["residue0"], xs)) < 1e-14
+
+
+@pytest.mark.parametrize("L", [(6, 6, 2, 2), (10, 6, 4, 4), (2, 2, 2, 2)])
+def test_max_shifts_on_ragged_lattices(stag, L):
+    """Edge cases: STAG_MAX_SHIFTS = 32 shifts (unsorted, with a duplicate), on lattices whose Vh (72, 480, 8)
+    is not a multiple of the warp, the CTA tile or the per-SM slice — empty CTAs and ragged tails everywhere."""
+    U, b, m = si.links_haar(L, 81), si.source_gaussian(L, 81), 0.2
+    shifts = [float(0.003 * 1.35 ** i) for i in range(stag.MAX_SHIFTS)]
+    shifts[5], shifts[20] = shifts[20], shifts[5]
+    shifts[7] = shifts[8]
+    ctx = stag.Stag(L)
+    packed = ctx.upload_gauge(U, 0, 18)
+    rc, info, xs, _ = gpu_cg(stag, ctx, packed, 0, 18, b, m, shifts, 1e-10, 5000)
+    ref = oracle.mshift_cg(L, U, b, m, shifts, 1e-10, 5000)
+    assert rc == 0 and abs(info["iters"] - ref["iters"]) <= 2
+    assert max(true_residuals(L, U, b, m, shifts, xs)) <= 1e-10
+    assert rel(xs[7], xs[8]) <= 1e-12
+    vb = ctx.vector_bytes(0)
+    assert ctx.cg_workspace_bytes(0, stag.MAX_SHIFTS + 1) == 0
+    with pytest.raises(stag.StagError):
+        ctx.mshift_cg(packed, 0, 18, ctx.upload_vector(b, 0), m, shifts + [1.0], 1e-10, 10, ctx.alloc(33 * vb),
+                      ctx.alloc(ctx.cg_workspace_bytes(0, 32)))

@@ -207,3 +207,35 @@ def test_c5_dslash_fp64_and_fp32_full_compare(stag, threads):
         ctx.dslash_oe(packed, prec, recon, vin, w)
         assert rel(ctx.download_vector(w, prec), want) <= TOL[prec], (prec, recon)
         del packed, vin, w
+
+
+@pytest.mark.parametrize("path", ["persistent", "multikernel"])
+def test_paper_shape_4x48cubed_cg_and_dslash(stag, threads, path):
+    """The paper's largest Table-2 lattice, 4 x 48^3: fp32 12-real Dslash (the paper's storage)
+    against the oracle, and the 8-shift fp64 solve on both CUDA paths — the persistent kernel runs here with
+    r and q resident and p_base in global memory (partial residency)."""
+    cfg = si.get_config("t2_48x48x48x4")
+    L, U, b, m, shifts, stop = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"], cfg["shifts"], cfg["stops"][0]
+    ctx = stag.Stag(L)
+    ctx.set_option("cg_persistent", 1 if path == "persistent" else 0)
+    if path == "persistent":
+        p32 = ctx.upload_gauge(U, 1, 12)
+        w = ctx.alloc(ctx.vector_bytes(1))
+        ctx.dslash_oe(p32, 1, 12, ctx.upload_vector(b, 1), w)
+        assert rel(ctx.download_vector(w, 1), oracle.dslash_oe(L, U, b)) <= 1e-5
+        del p32
+    packed = ctx.upload_gauge(U, 0, 18)
+    n, vb = len(shifts), ctx.vector_bytes(0)
+    x, ws = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(0, n))
+    rc, info = ctx.mshift_cg(packed, 0, 18, ctx.upload_vector(b, 0), m, shifts, stop, 100000, x, ws)
+    assert rc == 0, info
+    assert (info["kernel_launches"] == 1) == (path == "persistent")
+    nb = np.linalg.norm(b)
+    for i in (0, 3, 7):
+        xi = ctx.download_vector(x, 0, i * vb)
+        assert np.linalg.norm(b - oracle.apply_A(L, U, m, shifts[i], xi)) / nb <= stop
+    test_paper_shape_4x48cubed_cg_and_dslash.iters = getattr(test_paper_shape_4x48cubed_cg_and_dslash, "iters", {})
+    test_paper_shape_4x48cubed_cg_and_dslash.iters[path] = info["iters"]
+    it = test_paper_shape_4x48cubed_cg_and_dslash.iters
+    if len(it) == 2:
+        assert abs(it["persistent"] - it["multikernel"]) <= 2
