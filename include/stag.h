@@ -109,7 +109,9 @@ const char *stag_strerror(int err);
  * graph), "cg_freeze" (0|1: stop updating converged shifts, reading A10),
  * "cg_persistent" (1, default: lattices whose r, q, p_base slices fit in shared memory run the
  * whole solve as one cooperative kernel; 0: always the multi-kernel path),
- * "cg_persistent_threads" (0 auto | 256 | 512 | 1024 threads per CTA of that kernel). */
+ * "cg_persistent_threads" (0 auto | 256 | 512 | 1024 threads per CTA of that kernel),
+ * "cg_resident_slices" (0..3, default 3: how many of r, q, p_base the persistent kernel may keep in shared
+ * memory; fewer = the global-workspace path large lattices take). */
 int stag_set_option(stag_ctx *ctx, const char *key, int value);
 int stag_get_option(const stag_ctx *ctx, const char *key, int *value);
 

@@ -587,7 +587,9 @@ int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t
     a.S = sites_per_cta(g.Vh, grid);
     // residency: as many of r, q, p (in that order of bytes saved) as fit
     const size_t slice = (size_t)a.S * R * 6 * sizeof(T);
-    const int fit = (int)(kMaxDynSmem / slice);
+    // cg_resident_slices (test / tuning knob): cap on how many of r, q, p stay in shared memory (default 3)
+    int fit = (int)(kMaxDynSmem / slice);
+    if (fit > ctx->opt.cg_resident_slices) fit = ctx->opt.cg_resident_slices;
     a.res_r = fit >= 1; a.res_q = fit >= 2; a.res_p = fit >= 3;
     const size_t smem = slice * (size_t)(a.res_r + a.res_q + a.res_p);
     auto kern = cg_persistent_kernel<T, RECON, NT, R, SPLIT>;

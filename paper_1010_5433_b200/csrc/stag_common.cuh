@@ -62,6 +62,7 @@ struct Options {
     int cg_freeze;           // stop updating converged shifts (reading A10)
     int cg_ctas_per_sm;      // persistent grid size of the CG streaming kernels, per SM
     int cg_persistent_threads;  // persistent-kernel CTA: 1024 threads (64 regs) | 512 (128 regs) | 0 auto
+    int cg_resident_slices;  // persistent kernel: at most this many of r, q, p_base resident in shared memory (0..3)
     int cg_persistent;       // 1: whole solve as one cooperative kernel when r,q,p fit in shared memory; 0: never
 };
 

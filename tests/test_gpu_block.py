@@ -159,3 +159,34 @@ def test_block_badargs(stag):
             ctx.dslash_block(packed, 0, 18, 0, nrhs, v, w)
         assert ei.value.code == stag.ERR_BADARG
     assert ctx.cg_block_workspace_bytes(0, 4, 5) == 0
+
+
+@pytest.mark.parametrize("slices", [0, 1, 2, 3])
+@pytest.mark.parametrize("nrhs", [1, 3])
+@pytest.mark.parametrize("prec", [0, 1])
+def test_persistent_kernel_with_partial_residency(stag, slices, nrhs, prec):
+    """The persistent kernel keeps as many of r, q, p_base in shared memory as fit (all three on small lattices,
+    r and q at 4 x 48^3, r only for 4 sources at 32^3 x 8, none at 64^4).  cg_resident_slices forces each of the
+    four cases on a lattice the oracle solves in a moment; the result must not depend on it."""
+    L = (6, 4, 4, 8)
+    U, m, shifts = si.links_haar(L, 91), 0.1, [0.02, 0.3, 0.07, 1.1, 4.0]
+    bs = [si.source_gaussian(L, 91, stream=1 + k) for k in range(nrhs)]
+    stop = 1e-10 if prec == 0 else 1e-5
+    ctx = stag.Stag(L)
+    ctx.set_option("cg_resident_slices", slices)
+    packed = ctx.upload_gauge(U, prec, 18)
+    rc, infos, xs, _ = block_cg(stag, ctx, packed, prec, 18, bs, m, shifts, stop, 5000)
+    assert rc == 0
+    for s, b in enumerate(bs):
+        ref = oracle.mshift_cg(L, U, b, m, shifts, stop, 5000)
+        assert abs(infos[s]["iters"] - ref["iters"]) <= 2
+        nb = np.linalg.norm(b)
+        for i, sg in enumerate(shifts):
+            tr = np.linalg.norm(b - oracle.apply_A(L, U, m, sg, xs[s, i])) / nb
+            assert tr <= (stop if prec == 0 else 2e-4), (s, i, tr)
+    if nrhs == 1:                                         # the single-source ABI call takes the same kernel
+        vb = ctx.vector_bytes(prec)
+        x, ws = ctx.alloc(len(shifts) * vb), ctx.alloc(ctx.cg_workspace_bytes(prec, len(shifts)))
+        rc, info = ctx.mshift_cg(packed, prec, 18, ctx.upload_vector(bs[0], prec), m, shifts, stop, 5000, x, ws)
+        assert rc == 0 and info["kernel_launches"] == 1 and info["iters"] == infos[0]["iters"]
+        assert np.array_equal(ctx.download_vector(x, prec, 2 * vb), xs[0, 2])
