@@ -21,13 +21,13 @@ struct ForceCoef { double a[STAG_MAX_SHIFTS]; };
 // made each gather of X_i(z+mu) touch 4 lines per quarter-warp and the kernel sat at 74 % of
 // l1tex__data_pipe_lsu_wavefronts; one thread per site with all 4 directions needs 144 fp64 accumulators,
 // leaves 8 warps per SM and is latency-bound (12 % warps active).  Here a thread keeps one 3x3 sum (36
-// registers), which leaves room to unroll the shift loop by 4: 24 independent 16-byte loads in flight per
-// thread at 12+ warps per SM.  X_i(z) is requested by the 4 warps of a CTA (3 of the 4 hit L1).
+// registers), which leaves room to unroll the shift loop (fp64: x2 at 16 warps per SM; fp32: x4 at 12).
+// X_i(z) is requested by the 4 warps of a CTA (3 of the 4 hit L1).
 // The CTA's 32 x 576 contiguous output bytes leave through shared memory as full sectors.
 constexpr int kForceRow = 37;                          // 36 chunks of 16 B per site + 1 pad: conflict-free
 
-template <typename T, int RECON>
-__global__ void __launch_bounds__(128, 3)
+template <typename T, int RECON, int MINB, int UNR>
+__global__ void __launch_bounds__(128, MINB)
 force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ x_even,
              const char *__restrict__ w_odd, const size_t stride, const int nshift, const ForceCoef coef,
              double *__restrict__ force, const int accumulate) {
@@ -54,7 +54,7 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
         T m[18];
 #pragma unroll
         for (int k = 0; k < 18; ++k) m[k] = T(0);
-#pragma unroll 4
+#pragma unroll UNR
         for (int i = 0; i < nshift; ++i) {
             T a[6], b[6];
             load_vec(own + (size_t)i * stride, Vh, e, a);
@@ -145,9 +145,11 @@ extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int p
     for (int i = 0; i < STAG_MAX_SHIFTS; ++i) coef.a[i] = i < nshift ? host_residues[i] : 0.0;
     const dim3 grid((g.Vh + 31) / 32, 2), block(128);
     const char *W = static_cast<const char *>(packed);
-#define STAG_FORCE(T, R) force_kernel<T, R><<<grid, block, 0, st>>>(g, W, x, w, vbytes, nshift, coef, dev_force, accumulate)
-    if (prec == STAG_F64) { if (recon == 18) STAG_FORCE(double, 18); else STAG_FORCE(double, 12); }
-    else { if (recon == 18) STAG_FORCE(float, 18); else STAG_FORCE(float, 12); }
+    // occupancy / unroll measured at 32^3 x 8, 16 shifts (profiles/README.md "N4"): fp64 is fastest with 128
+    // registers (16 warps per SM) and the shift loop unrolled x2, fp32 with 3 CTAs per SM and x4
+#define STAG_FORCE(T, R, M, U) force_kernel<T, R, M, U><<<grid, block, 0, st>>>(g, W, x, w, vbytes, nshift, coef, dev_force, accumulate)
+    if (prec == STAG_F64) { if (recon == 18) STAG_FORCE(double, 18, 4, 2); else STAG_FORCE(double, 12, 4, 2); }
+    else { if (recon == 18) STAG_FORCE(float, 18, 3, 4); else STAG_FORCE(float, 12, 3, 4); }
 #undef STAG_FORCE
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
