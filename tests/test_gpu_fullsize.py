@@ -239,3 +239,26 @@ def test_paper_shape_4x48cubed_cg_and_dslash(stag, threads, path):
     it = test_paper_shape_4x48cubed_cg_and_dslash.iters
     if len(it) == 2:
         assert abs(it["persistent"] - it["multikernel"]) <= 2
+
+
+def test_32x32cubed_block_cg_nothing_resident(stag, threads):
+    """The paper's 32 x 32^3 lattice, two sources in one persistent launch: at this size no slice
+    of r, q, p fits in shared memory (every vector goes through the global workspace) and the single-source call
+    takes the multi-kernel path; both must give the oracle's residuals and the same iteration count +-2."""
+    cfg = si.get_config("t2_32x32x32x32")
+    L, U, m, shifts, stop = cfg["L"], si.make_links(cfg), cfg["mass"], cfg["shifts"], cfg["stops"][0]
+    bs = [si.source_gaussian(L, cfg["seed"], stream=1 + k) for k in range(2)]
+    ctx = stag.Stag(L)
+    packed = ctx.upload_gauge(U, 0, 18)
+    n, vb = len(shifts), ctx.vector_bytes(0)
+    x, ws = ctx.alloc(2 * n * vb), ctx.alloc(ctx.cg_block_workspace_bytes(0, n, 2))
+    rc, infos = ctx.mshift_cg_block(packed, 0, 18, 2, ctx.upload_vectors(bs, 0), m, shifts, stop, 100000, x, ws)
+    assert rc == 0 and infos[0]["kernel_launches"] == 1
+    x1, ws1 = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(0, n))
+    rc, info = ctx.mshift_cg(packed, 0, 18, ctx.upload_vector(bs[0], 0), m, shifts, stop, 100000, x1, ws1)
+    assert rc == 0 and info["kernel_launches"] > 1 and abs(info["iters"] - infos[0]["iters"]) <= 2
+    for s, i in ((0, 0), (1, 0), (1, n - 1)):
+        xi = ctx.download_vector(x, 0, (s * n + i) * vb)
+        assert np.linalg.norm(bs[s] - oracle.apply_A(L, U, m, shifts[i], xi)) / np.linalg.norm(bs[s]) <= stop
+    xi = ctx.download_vector(x1, 0, 0)
+    assert np.linalg.norm(bs[0] - oracle.apply_A(L, U, m, shifts[0], xi)) / np.linalg.norm(bs[0]) <= stop
