@@ -15,7 +15,7 @@ namespace stag {
 
 struct ForceCoef { double a[STAG_MAX_SHIFTS]; };
 
-// CTA = 32 consecutive sites of parity blockIdx.y x 4 directions; thread = one link (z, mu) with mu = the
+// CTA = 32 consecutive sites of one parity x 4 directions; thread = one link (z, mu) with mu = the
 // WARP index, so every 128-bit load instruction of a warp covers 32 consecutive sites (one 128-byte line per
 // quarter-warp).  Two earlier mappings, both measured (profiles/README.md, N4): mu as the fastest LANE index
 // made each gather of X_i(z+mu) touch 4 lines per quarter-warp and the kernel sat at 74 % of
@@ -33,8 +33,11 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
              double *__restrict__ force, const int accumulate) {
     __shared__ double2 stage[32 * kForceRow];          // [site][mu][9 complex] (+ pad)
     __shared__ int s_lex[32];
-    const int mu = threadIdx.x >> 5, ls = threadIdx.x & 31, par = blockIdx.y;
-    const int e = blockIdx.x * 32 + ls;
+    const int mu = threadIdx.x >> 5, ls = threadIdx.x & 31;
+    // consecutive CTAs alternate parity over the same 32-site tile: the X_i one reads as X_i(z) the other reads
+    // as X_i(z+mu) a moment later, out of L2 (measured: 316 -> 305 us per fp64 call)
+    const int par = blockIdx.x & 1, tile = blockIdx.x >> 1;
+    const int e = tile * 32 + ls;
     const int Vh = g.Vh;
     if (e < Vh) {
         const Site s = site_of(g, e, par);
@@ -104,7 +107,7 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
     }
     __syncthreads();
     // 32 sites x 36 chunks of 16 bytes; consecutive threads write consecutive chunks of one site
-    const int nsite = min(32, Vh - (int)blockIdx.x * 32);
+    const int nsite = min(32, Vh - tile * 32);
     for (int k = threadIdx.x; k < nsite * 36; k += 128) {
         const int site = k / 36, c = k - site * 36;
         double2 v = stage[site * kForceRow + c];
@@ -143,7 +146,7 @@ extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int p
     }
     ForceCoef coef;
     for (int i = 0; i < STAG_MAX_SHIFTS; ++i) coef.a[i] = i < nshift ? host_residues[i] : 0.0;
-    const dim3 grid((g.Vh + 31) / 32, 2), block(128);
+    const dim3 grid(2 * ((g.Vh + 31) / 32)), block(128);
     const char *W = static_cast<const char *>(packed);
     // occupancy / unroll measured at 32^3 x 8, 16 shifts (profiles/README.md "N4"): fp64 is fastest with 128
     // registers (16 warps per SM) and the shift loop unrolled x2, fp32 with 3 CTAs per SM and x4
