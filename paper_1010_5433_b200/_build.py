@@ -12,6 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libstag_b200.so")
+SO_TIMERS = os.path.join(HERE, "libstag_b200_timers.so")     # -DSTAG_PHASE_TIMERS build (STAG_PHASE_TIMERS=1)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 OBJ = os.path.join(HERE, "build")
@@ -33,13 +34,20 @@ def stale() -> bool:
     return any(os.path.getmtime(f) > t for f in _deps())
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, timers: bool = False) -> str:
+    """timers=True: the per-phase-timer build of the persistent CG (csrc/stag_cg_persist.cuh), a separate .so."""
+    if timers:
+        return _build(SO_TIMERS, ["-DSTAG_PHASE_TIMERS"], verbose)
     if not force and not stale():
         return SO
+    return _build(SO, [], verbose)
+
+
+def _build(SO: str, defines: list[str], verbose: bool) -> str:
     from concurrent.futures import ThreadPoolExecutor
     nvcc = os.environ.get("NVCC", "nvcc")
     os.makedirs(OBJ, exist_ok=True)
-    extra = ["-Xptxas", "-v"] if verbose else []
+    extra = (["-Xptxas", "-v"] if verbose else []) + defines
 
     def compile_one(src: str) -> str:          # one translation unit per worker: seconds, not a minute
         obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".%d.o" % os.getpid())
@@ -57,4 +65,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv,
+                timers=os.environ.get("STAG_PHASE_TIMERS") == "1"))

@@ -35,6 +35,36 @@
 #include "stag_cg.cuh"
 #include "stag_dslash.cuh"
 
+// Per-phase timers (build with -DSTAG_PHASE_TIMERS: `STAG_PHASE_TIMERS=1 python -m paper_1010_5433_b200._build`
+// writes libstag_b200_timers.so, which the binding loads when the same variable is set).  CTAs 0, 77 and the last
+// one print, at the end of the solve, the mean microseconds per iteration they spent in each phase and in each
+// grid-barrier wait (%globaltimer, CTA-wide: a __syncthreads precedes every tick).  Compiles to nothing otherwise.
+#ifdef STAG_PHASE_TIMERS
+#include <cstdio>
+#define STAG_T_DECL                                                                       \
+    unsigned long long tt_[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, t0_, t1_;                    \
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0_));
+#define STAG_TICK(k)                                                                      \
+    do {                                                                                  \
+        __syncthreads();                                                                  \
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1_));                           \
+        tt_[k] += t1_ - t0_;                                                              \
+        t0_ = t1_;                                                                        \
+    } while (0)
+#define STAG_T_REPORT(R_, iters_)                                                                          \
+    if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == gridDim.x - 1)) {       \
+        const double k_ = 1e-3 / ((iters_) > 0 ? (iters_) : 1);                                            \
+        printf("[stag timers] CTA %d R=%d iters %d  us/iter: A %.2f wait %.2f | B %.2f wait %.2f | C %.2f " \
+               "wait %.2f | D base %.2f shifts %.2f wait %.2f\n", (int)blockIdx.x, R_, (int)(iters_),      \
+               tt_[0] * k_, tt_[1] * k_, tt_[2] * k_, tt_[3] * k_, tt_[4] * k_, tt_[5] * k_, tt_[6] * k_,  \
+               tt_[7] * k_, tt_[8] * k_);                                                                  \
+    }
+#else
+#define STAG_T_DECL
+#define STAG_TICK(k) ((void)0)
+#define STAG_T_REPORT(R_, iters_)
+#endif
+
 namespace stag {
 
 // ---- grid barrier: monotone counter, arrive / wait split ---------------------------------------
@@ -327,6 +357,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
     }
 
     // ---- iterations -----------------------------------------------------------------------------------
+    STAG_T_DECL
     while (n_running > 0) {
         const bool act = sc[rhs].done == 0;          // streaming phases: this thread's source is still iterating
         unsigned mask = 0;                           // stencil phases: the sources still iterating
@@ -341,8 +372,10 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             for (int r = 0; r < R; ++r)
                 if (R == 1 || ((mask >> r) & 1u)) store_vec(wout[r], Vh, e0 + ls, acc[r]);
         }
+        STAG_TICK(0);
         grid_arrive(bar);
         grid_wait(bar, ++epoch * G);
+        STAG_TICK(1);
 
         // phase B (a3): q = c0 p - D_eo w, partial Re<p,q>
         {
@@ -369,8 +402,10 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             }
             cta_partials_all<NT, R>(dot, red, part_pq + blockIdx.x, G);
         }
+        STAG_TICK(2);
         grid_arrive(bar);
         grid_wait(bar, ++epoch * G);
+        STAG_TICK(3);
 
         // phase C (a4 after <p,q>, then a5): alpha, theta_new_i;  r -= alpha q;  partial <r,r>
         if (tid < 32 * R) {
@@ -413,8 +448,10 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             }
             cta_partials_stream<NT, R>(acc, red, part_rr + blockIdx.x, G);
         }
+        STAG_TICK(4);
         grid_arrive(bar);
         grid_wait(bar, ++epoch * G);
+        STAG_TICK(5);
 
         // phase D (a4 after <r,r>, a7 latch, a6)
         if (tid < 32 * R) {
@@ -489,6 +526,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                 store_vec(p_base, Vh, e, pv);
             }
         }
+        STAG_TICK(6);
         grid_arrive(bar);
         if (act2) {
             const Scalars<T> &c = sc[rhs];
@@ -524,8 +562,12 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             }
             n_running = n;
         }
+        STAG_TICK(7);
         grid_wait(bar, ++epoch * G);                   // ends with __syncthreads: n_running, done visible
+        STAG_TICK(8);
     }
+
+    STAG_T_REPORT(R, sc[0].iter)
 
     // ---- a7: y = residue0 b + sum_i residues_i x_i (own sites only: no barrier needed) ---------------
     if (a.y && present) {
