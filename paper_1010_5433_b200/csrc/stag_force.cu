@@ -52,6 +52,16 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
             const T eta = (phase_sum & 1) ? T(-2) : T(2);
             c3 = (mu == 3 && x[3] == Lmu - 1) ? -eta : eta;
         }
+        // the matrix is needed only after the shift loop: ask L2 for its lines now (no registers held), so the
+        // load after the loop is an L2 hit instead of one more DRAM latency on every CTA's critical path
+        {
+            const size_t set_ = link_set_bytes<T, RECON>(Vh);
+            const char *wl = W + (size_t)(par * 8 + 2 * mu) * set_ + (size_t)e * 16;
+            constexpr int NCH = (RECON * (int)sizeof(T) + 15) / 16;
+#pragma unroll
+            for (int k = 0; k < NCH; ++k)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(wl + (size_t)k * Vh * 16));
+        }
         const char *own = (par == 0 ? x_even : w_odd);     // X_i(z)
         const char *nbr = (par == 0 ? w_odd : x_even);     // X_i(z + mu)
         T m[18];
