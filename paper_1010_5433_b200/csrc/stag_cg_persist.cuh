@@ -82,7 +82,8 @@ __device__ __forceinline__ void grid_wait(unsigned int *bar, unsigned int target
         do {
             asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
         } while ((int)(v - target) < 0);
-        __threadfence();
+        // the acquire load orders everything after it (and, through the CTA barrier below, every other
+        // thread's later loads) behind the arrivals it observed: no further fence needed
     }
     __syncthreads();
 }
