@@ -324,6 +324,28 @@ def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
                      "true_resid_after_fp32": max(info["polish"]["resid_before"]),
                      "true_resid_final": max(info["polish"]["resid_after"]),
                      "kernel_launches": info["inner"]["kernel_launches"] + info["polish"]["kernel_launches"]}
+    # single shift (the lightest): the inner stage is the persistent residual-replacement kernel and stops on the
+    # TRUE fp64 residual, nothing is left to polish; the fp64 solver on the same single system beside it
+    sh1 = cfg["shifts"][:1]
+    cgws = ctx.alloc(ctx.cg_workspace_bytes(stag.F64, 1))
+    for _ in range(2):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        rc64, i64 = ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], sh1, cfg["stops"][0], 100000, x, cgws)
+        e1.record()
+        torch.cuda.synchronize()
+    t64 = e0.elapsed_time(e1) * 1e-3
+    for _ in range(2):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        rc, info = ctx.mshift_cg_mixed(p64, stag.F64, 18, split, 18, b, cfg["mass"], sh1, cfg["stops"][0], 100000, x, ws)
+        e1.record()
+        torch.cuda.synchronize()
+    tm = e0.elapsed_time(e1) * 1e-3
+    out["single_shift_residual_replacement"] = {
+        "rc": rc, "s_per_solve": tm, "fp64_s_per_solve": t64, "vs_fp64": t64 / tm, "iters": info["inner"]["iters"],
+        "fp64_iters": i64["iters"], "reliable_updates": info["reliable_updates"],
+        "polish_iters": sum(info["polish"]["iters"]), "true_resid_final": info["polish"]["resid_after"][0]}
     return out
 
 

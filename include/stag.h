@@ -110,6 +110,9 @@ const char *stag_strerror(int err);
  * "cg_persistent" (1, default: lattices whose r, q, p_base slices fit in shared memory run the
  * whole solve as one cooperative kernel; 0: always the multi-kernel path),
  * "cg_persistent_threads" (0 auto | 256 | 512 | 1024 threads per CTA of that kernel),
+ * "cg_mixed_reliable" (stag_mshift_cg_mixed: run the inner stage as the persistent kernel with residual
+ * replacement — 0 never | 1, default: single-shift solves | 2 always), "cg_mixed_delta_inv" (>= 2, default 10:
+ * replace the residual whenever ||r|| has fallen by this factor),
  * "cg_resident_slices" (0..3, default 3: how many of r, q, p_base the persistent kernel may keep in shared
  * memory; fewer = the global-workspace path large lattices take). */
 int stag_set_option(stag_ctx *ctx, const char *key, int value);
@@ -207,8 +210,9 @@ typedef struct stag_polish_info {
     int kernel_launches;
 } stag_polish_info;
 typedef struct stag_mixed_info {
-    stag_cg_info inner;                      /* the fp32 multi-shift run                                  */
+    stag_cg_info inner;                      /* the inner (fp32-matrix) multi-shift run                   */
     stag_polish_info polish;
+    int reliable_updates;                    /* residual replacements of the inner run (0: plain fp32 run) */
 } stag_mixed_info;
 
 /* dst = src converted between device vector formats (nvec contiguous vectors each side). */
@@ -224,7 +228,12 @@ int stag_cg_polish(const stag_ctx *ctx, const void *packed, int prec, int recon,
                    double mass, int nshift, const double *host_shifts, double stop, int maxiter,
                    void *x_even, void *workspace, stag_polish_info *info, void *stream);
 
-/* fp32 multi-shift CG to inner_stop (<= 0: default 1e-5) on packed_lo (STAG_F32 format — e.g. the first
+/* Inner stage, then the polish, then y.  Inner stage, single shift with prec_hi = STAG_F64 and recon_hi =
+ * recon_lo (option "cg_mixed_reliable"): ONE persistent kernel with RESIDUAL REPLACEMENT (ref [7]):
+ * fp32 matrices, r, q, p; x in fp64; whenever ||r|| has fallen tenfold, and again at stop, the true residual
+ * b - (A + sigma) x is recomputed with the fp64 matrices and replaces the recursive one; convergence is declared
+ * on that true residual, so the polish has nothing left to do.  Otherwise:
+ * fp32 multi-shift CG to inner_stop (<= 0: default 1e-5) on packed_lo (STAG_F32 format — e.g. the first
  * half of a STAG_F64_SPLIT buffer), then the polish on packed_hi (prec_hi = STAG_F64 | STAG_F64_SPLIT) to
  * stop, then y.  b_even, x_even, y_even: fp64 device format.  The fp32 stage ending on stagnation or
  * maxiter is not an error: the polish finishes the job.  Returns as stag_cg_polish. */

@@ -36,6 +36,8 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
     c->opt.cg_persistent = 1;
     c->opt.cg_persistent_threads = 0;
     c->opt.cg_resident_slices = 3;
+    c->opt.cg_mixed_reliable = 1;
+    c->opt.cg_mixed_delta_inv = 10;
     if (cudaGetDevice(&c->device) != cudaSuccess ||
         cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess ||
         cudaHostAlloc((void **)&c->pinned_flags, 512, cudaHostAllocMapped) != cudaSuccess ||
@@ -81,6 +83,8 @@ static int *option_slot(Options &o, const char *key) {
     if (!std::strcmp(key, "cg_persistent")) return &o.cg_persistent;
     if (!std::strcmp(key, "cg_persistent_threads")) return &o.cg_persistent_threads;
     if (!std::strcmp(key, "cg_resident_slices")) return &o.cg_resident_slices;
+    if (!std::strcmp(key, "cg_mixed_reliable")) return &o.cg_mixed_reliable;
+    if (!std::strcmp(key, "cg_mixed_delta_inv")) return &o.cg_mixed_delta_inv;
     return nullptr;
 }
 
@@ -94,6 +98,8 @@ extern "C" int stag_set_option(stag_ctx *ctx, const char *key, int value) {
         return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_check_every && value < 1) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_persistent_threads && value != 0 && value != 256 && value != 512 && value != 1024) return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.cg_mixed_delta_inv && value < 2) return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.cg_mixed_reliable && (value < 0 || value > 2)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_resident_slices && (value < 0 || value > 3)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_ctas_per_sm && (value < 1 || value > 16)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.dslash_ctas_per_sm && (value < 0 || value > 32)) return STAG_ERR_BADARG;

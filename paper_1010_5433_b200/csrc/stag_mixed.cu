@@ -8,7 +8,7 @@
 #include <cmath>
 #include <cstring>
 
-#include "stag_cg.cuh"
+#include "stag_cg_mixed_persist.cuh"
 
 namespace stag {
 
@@ -218,7 +218,7 @@ partial_fraction64_kernel(const long nchunk, const double2 *__restrict__ b, cons
     }
 }
 
-struct MixedLayout { size_t res, b32, x32, cg32, polish, total; };
+struct MixedLayout { size_t res, b32, x32, cg32, w64, polish, total; };
 
 static MixedLayout mixed_layout(const stag_ctx *ctx, int nshift) {
     MixedLayout l;
@@ -228,9 +228,65 @@ static MixedLayout mixed_layout(const stag_ctx *ctx, int nshift) {
     l.b32 = off;    off += align256(v32);
     l.x32 = off;    off += align256(v32 * (size_t)nshift);
     l.cg32 = off;   off += align256(cg_workspace_layout(ctx, STAG_F32, nshift, nullptr));
+    l.w64 = off;    off += align256((size_t)ctx->g.Vh * vec_bytes_per_site(STAG_F64));
     l.polish = off; off += polish_layout(ctx).total;
     l.total = off;
     return l;
+}
+
+// The inner stage as ONE persistent kernel with residual replacement (stag_cg_mixed_persist.cuh): fp32 matrices
+// and directions, fp64 solutions, true fp64 residual of the base system at every replacement.  Returns
+// STAG_ERR_UNSUPPORTED when that kernel does not apply (the caller then runs the plain fp32 stage).
+static int mixed_persistent(const stag_ctx *ctx, const void *packed_hi, const void *packed_lo, int recon,
+                            const void *b64, double mass, int nshift, const double *shifts, double stop,
+                            int maxiter, void *x64, char *ws, const MixedLayout &lay, stag_cg_info *info,
+                            int *replacements, cudaStream_t st) {
+    if (!cg_persistent_fits(ctx, STAG_F32)) return STAG_ERR_UNSUPPORTED;
+    CgLayout cl;
+    cg_workspace_layout(ctx, STAG_F32, nshift, &cl);
+    char *cw = ws + lay.cg32;
+    int base = 0;
+    for (int i = 1; i < nshift; ++i)
+        if (shifts[i] < shifts[base]) base = i;
+    CgState *h = static_cast<CgState *>(ctx->pinned_info);
+    std::memset(h, 0, sizeof(*h));
+    h->alpha_old = 1.0;
+    h->c0 = mass * mass + shifts[base];
+    h->stop = stop;
+    for (int i = 0; i < nshift; ++i) {
+        h->delta[i] = shifts[i] - shifts[base];
+        h->zeta[i] = 1.0; h->theta[i] = 1.0; h->active[i] = 1; h->resid_shift[i] = 1.0;
+    }
+    h->nshift = nshift; h->base = base; h->maxiter = maxiter; h->freeze = ctx->opt.cg_freeze; h->fp32 = 1;
+    STAG_CUDA_OK(cudaMemcpyAsync(cw + cl.state, h, sizeof(CgState), cudaMemcpyHostToDevice, st));
+    MixedArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.W_lo = static_cast<const char *>(packed_lo);
+    a.W_hi = static_cast<const char *>(packed_hi);
+    a.b64 = static_cast<const char *>(b64);
+    a.w32 = cw + cl.w; a.w64 = ws + lay.w64;
+    a.r_g = cw + cl.r; a.q_g = cw + cl.q;
+    a.p = cw + cl.p; a.p_stride = cl.vec_stride;
+    a.x = static_cast<char *>(x64); a.x_stride = (size_t)ctx->g.Vh * vec_bytes_per_site(STAG_F64);
+    a.state = reinterpret_cast<CgState *>(cw + cl.state);
+    a.partials = reinterpret_cast<double *>(cw + cl.partials);
+    a.ru_delta = 1.0 / (double)(ctx->opt.cg_mixed_delta_inv > 0 ? ctx->opt.cg_mixed_delta_inv : 10);
+    const int nt = ctx->opt.cg_persistent_threads;
+    int rc = recon == 18 ? (nt == 512 ? launch_mixed<18, 512>(ctx, a, st) : launch_mixed<18, 1024>(ctx, a, st))
+                         : (nt == 512 ? launch_mixed<12, 512>(ctx, a, st) : launch_mixed<12, 1024>(ctx, a, st));
+    if (rc) { cudaGetLastError(); return rc; }
+    STAG_CUDA_OK(cudaMemcpyAsync(h, cw + cl.state, sizeof(CgState), cudaMemcpyDeviceToHost, st));
+    STAG_CUDA_OK(cudaStreamSynchronize(st));
+    std::memset(info, 0, sizeof(*info));
+    info->iters = h->iter; info->converged = h->converged; info->breakdown = h->breakdown;
+    info->bnorm2 = h->bb; info->rnorm2 = h->rr; info->kernel_launches = 1;
+    for (int i = 0; i < nshift; ++i) {
+        info->resid_iter[i] = h->bb > 0.0 ? h->resid_shift[i] : 0.0;
+        info->iters_shift[i] = h->iters_shift[i];
+    }
+    *replacements = h->since_best;
+    if (h->breakdown) return STAG_ERR_BREAKDOWN;
+    return h->converged ? STAG_OK : STAG_ERR_NOTCONV;
 }
 
 }  // namespace stag
@@ -307,8 +363,23 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     stag_mixed_info mi;
     std::memset(&mi, 0, sizeof(mi));
 
-    // fp32 stage: b -> fp32, multi-shift CG from zero, x -> fp64
-    int rc = stag_vector_convert(ctx, b_even, STAG_F64, ws + lay.b32, STAG_F32, 1, st);
+    // inner stage, preferred form: one persistent kernel with residual replacement (fp32 matrices, fp64 x_i)
+    int rc = STAG_ERR_UNSUPPORTED;
+    // cg_mixed_reliable: 0 never | 1 (default) when it pays — a single shift, where nothing is left to polish
+    // (32^3 x 8: 0.107 s against 0.169 s in fp64; with more shifts the shifted systems stop at the fp32
+    // rounding of the matrices times ||x_i||/||b|| and the polish costs as much as after the plain fp32 run) | 2 always
+    const bool want_ru = ctx->opt.cg_mixed_reliable == 2 || (ctx->opt.cg_mixed_reliable == 1 && nshift == 1);
+    if (want_ru && ctx->opt.cg_persistent && prec_hi == STAG_F64 && recon_hi == recon_lo)
+        rc = mixed_persistent(ctx, packed_hi, packed_lo, recon_lo, b_even, mass, nshift, host_shifts, stop, maxiter,
+                              x_even, ws, lay, &mi.inner, &mi.reliable_updates, st);
+    if (rc != STAG_ERR_UNSUPPORTED) {
+        if (rc != STAG_OK && rc != STAG_ERR_NOTCONV) {
+            if (info) *info = mi;
+            return rc;
+        }
+    } else {
+    // plain fp32 stage: b -> fp32, multi-shift CG from zero, x -> fp64
+    rc = stag_vector_convert(ctx, b_even, STAG_F64, ws + lay.b32, STAG_F32, 1, st);
     if (rc) return rc;
     rc = stag_mshift_cg(ctx, packed_lo, STAG_F32, recon_lo, ws + lay.b32, mass, nshift, host_shifts, nullptr, 0.0,
                         inner_stop, maxiter, ws + lay.x32, nullptr, ws + lay.cg32, &mi.inner, st);
@@ -318,6 +389,7 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     }
     rc = stag_vector_convert(ctx, ws + lay.x32, STAG_F32, x_even, STAG_F64, nshift, st);
     if (rc) return rc;
+    }
 
     // fp64 stage: per-shift defect-correction polish
     const int prc = polish(ctx, packed_hi, prec_hi, recon_hi, static_cast<const char *>(b_even), mass, nshift,

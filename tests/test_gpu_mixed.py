@@ -87,11 +87,17 @@ def test_polish_from_shared_start_matches_oracle_polish(stag, prec_name, recon, 
             assert ref["iters"] - 2 <= info["iters"][i] <= ref["iters"] + 12      # a second pass adds a few
 
 
-@pytest.mark.parametrize("hi,recon_hi,recon_lo", [("F64", 18, 18), ("F64", 12, 12), ("F64_SPLIT", 18, 18)])
-def test_mixed_config1(stag, hi, recon_hi, recon_lo):
+@pytest.mark.parametrize("hi,recon_hi,recon_lo,reliable", [("F64", 18, 18, 2), ("F64", 12, 12, 2), ("F64", 18, 18, 1),
+                                                           ("F64", 18, 12, 2), ("F64_SPLIT", 18, 18, 2)])
+def test_mixed_config1(stag, hi, recon_hi, recon_lo, reliable):
+    """reliable = 2 (forced; the default 1 uses it for single-shift solves only) with native fp64 matrices of the same recon: the inner stage is the persistent kernel with
+    residual replacement (fp32 matrices, fp64 x_i, convergence on the TRUE fp64 residual of the base system);
+    otherwise (option off, split-double, different recon) the plain fp32 stage + polish."""
     cfg = si.get_config("c1_4x4x4x4")
     L, U, b, m, shifts = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"], cfg["shifts"]
     ctx = stag.Stag(L)
+    ctx.set_option("cg_mixed_reliable", reliable)
+    replaced = reliable == 2 and hi == "F64" and recon_hi == recon_lo
     prec_hi = getattr(stag, hi)
     p_hi = ctx.upload_gauge(U, prec_hi, recon_hi)
     p_lo = p_hi if hi == "F64_SPLIT" else ctx.upload_gauge(U, stag.F32, recon_lo)   # N3: one buffer, both precisions
@@ -102,16 +108,53 @@ def test_mixed_config1(stag, hi, recon_hi, recon_lo):
     rc, info = ctx.mshift_cg_mixed(p_hi, prec_hi, recon_hi, p_lo, recon_lo, ctx.upload_vector(b, stag.F64), m,
                                    shifts, 1e-10, 2000, x, ws, residues=residues, residue0=2.0, y_even=y)
     assert rc == 0, info
-    assert info["inner"]["iters"] > 0 and max(info["polish"]["iters"]) > 0
+    ref = oracle.mshift_cg(L, U, b, m, shifts, 1e-10, 2000)
+    if replaced:
+        assert info["reliable_updates"] >= 2 and info["inner"]["converged"] and info["inner"]["kernel_launches"] == 1
+        assert info["polish"]["resid_before"][shifts.index(min(shifts))] <= 1e-10     # converged on the true residual
+        # the shifted systems ride along: their floor is the fp32 rounding of the matrices times ||x_i|| / ||b||
+        assert max(info["polish"]["resid_before"]) <= 1e-5
+        assert abs(info["inner"]["iters"] - ref["iters"]) <= max(10, ref["iters"] // 5)
+    else:
+        assert info["reliable_updates"] == 0
+        assert info["inner"]["iters"] > 0 and max(info["polish"]["iters"]) > 0
     A = oracle.dense_A(L, U, m)
     xs = []
     for i, s in enumerate(shifts):
         xi = ctx.download_vector(x, stag.F64, i * vb)
         xs.append(xi)
-        assert 1e-9 < info["polish"]["resid_before"][i] < 1e-2          # what fp32 alone reached
+        if not replaced:
+            assert 1e-9 < info["polish"]["resid_before"][i] < 1e-2      # what fp32 alone reached
         assert true_res(L, U, m, s, b, xi) <= 1e-10
         assert rel(xi, oracle.dense_solve(A, s, b).reshape(-1, 3)) <= 1e-8
     assert rel(ctx.download_vector(y, stag.F64), oracle.partial_fraction(b, residues, 2.0, np.stack(xs))) <= 1e-14
+
+
+@pytest.mark.parametrize("slices", [3, 1, 0])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_mixed_single_shift_residual_replacement(stag, slices, recon):
+    """Single shift, default options: the inner stage is the persistent residual-replacement kernel; it must stop
+    on the TRUE residual (nothing left to polish), in about as many iterations as the fp64 oracle, in every
+    shared-memory residency case."""
+    cfg = si.get_config("c2_16x16x16x4")
+    L, U, b, m, shifts = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"], cfg["shifts"]
+    ctx = stag.Stag(L)
+    ctx.set_option("cg_resident_slices", slices)
+    p64, p32 = ctx.upload_gauge(U, stag.F64, recon), ctx.upload_gauge(U, stag.F32, recon)
+    vb = ctx.vector_bytes(stag.F64)
+    x, ws = ctx.alloc(vb), ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(1))
+    x.fill_(0xFF)
+    rc, info = ctx.mshift_cg_mixed(p64, stag.F64, recon, p32, recon, ctx.upload_vector(b, stag.F64), m, shifts,
+                                   1e-10, 20000, x, ws)
+    ref = oracle.mshift_cg(L, U, b, m, shifts, 1e-10, 20000)
+    assert rc == 0 and info["inner"]["converged"] and info["inner"]["kernel_launches"] == 1, info
+    assert info["reliable_updates"] >= 5 and sum(info["polish"]["iters"]) == 0 and info["polish"]["passes"] == 0
+    assert abs(info["inner"]["iters"] - ref["iters"]) <= max(3, ref["iters"] // 10)
+    assert true_res(L, U, m, shifts[0], b, ctx.download_vector(x, stag.F64)) <= 1e-10
+    # maxiter reached: reports NOTCONV with the true residual it got to
+    rc, info = ctx.mshift_cg_mixed(p64, stag.F64, recon, p32, recon, ctx.upload_vector(b, stag.F64), m, shifts,
+                                   1e-10, 5, x, ws)
+    assert rc == stag.ERR_NOTCONV and info["inner"]["iters"] == 5 and info["polish"]["resid_after"][0] > 1e-10
 
 
 def test_mixed_config2_single_shift(stag):
