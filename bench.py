@@ -338,7 +338,8 @@ def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
     for _ in range(2):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        rc, info = ctx.mshift_cg_mixed(p64, stag.F64, 18, split, 18, b, cfg["mass"], sh1, cfg["stops"][0], 100000, x, ws)
+        # fp32 iterations on the b planes, fp64 residual replacement on b + c of the SAME split-double buffer (N3)
+        rc, info = ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], sh1, cfg["stops"][0], 100000, x, ws)
         e1.record()
         torch.cuda.synchronize()
     tm = e0.elapsed_time(e1) * 1e-3

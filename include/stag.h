@@ -228,7 +228,7 @@ int stag_cg_polish(const stag_ctx *ctx, const void *packed, int prec, int recon,
                    double mass, int nshift, const double *host_shifts, double stop, int maxiter,
                    void *x_even, void *workspace, stag_polish_info *info, void *stream);
 
-/* Inner stage, then the polish, then y.  Inner stage, single shift with prec_hi = STAG_F64 and recon_hi =
+/* Inner stage, then the polish, then y.  Inner stage, single shift with recon_hi =
  * recon_lo (option "cg_mixed_reliable"): ONE persistent kernel with RESIDUAL REPLACEMENT (ref [7]):
  * fp32 matrices, r, q, p; x in fp64; whenever ||r|| has fallen tenfold, and again at stop, the true residual
  * b - (A + sigma) x is recomputed with the fp64 matrices and replaces the recursive one; convergence is declared

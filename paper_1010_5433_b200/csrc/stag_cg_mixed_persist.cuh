@@ -23,7 +23,7 @@
 namespace stag {
 
 struct MixedArgs {
-    const char *W_lo, *W_hi;   // packed hopping matrices: fp32 and fp64 (same recon)
+    const char *W_lo, *W_hi;   // packed hopping matrices: fp32 and fp64 or split-double (same recon)
     const char *b64;           // source, fp64 device format
     char *w32, *w64;           // odd-site scratch: fp32 (every iteration), fp64 (residual replacement)
     char *r_g, *q_g;           // global homes of r, q (fp32) when not resident
@@ -44,7 +44,8 @@ struct MixedExtra {            // scalars the mixed kernel needs on top of Scala
     int ru, verify, nru, last;
 };
 
-template <int RECON, int NT>
+// SPLIT_HI: W_hi is a split-double buffer (N3) — typically the very buffer whose b planes are W_lo.
+template <int RECON, int NT, bool SPLIT_HI>
 __global__ void __launch_bounds__(NT, 1)
 cg_mixed_kernel(const Geom g, const MixedArgs a) {
     typedef float T;
@@ -130,7 +131,7 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
         if (mx.ru) {
             for (int ls = tid; ls < ns; ls += NT) {
                 double acc[1][6];
-                dslash_site_multi<double, RECON, 1, false>(g, a.W_hi, xin64, 1u, 1, e0 + ls, acc);
+                dslash_site_multi<double, RECON, 1, false, SPLIT_HI>(g, a.W_hi, xin64, 1u, 1, e0 + ls, acc);
                 store_vec(a.w64, Vh, e0 + ls, acc[0]);
             }
             grid_arrive(bar);
@@ -141,7 +142,7 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
                 const int e = e0 + ls;
                 double t[1][6], xv[6], bv[6];
                 T rv[6];
-                dslash_site_multi<double, RECON, 1, false>(g, a.W_hi, win64, 1u, 0, e, t);
+                dslash_site_multi<double, RECON, 1, false, SPLIT_HI>(g, a.W_hi, win64, 1u, 0, e, t);
                 load_vec<false>(x_base, Vh, e, xv);
                 load_vec<true>(a.b64, Vh, e, bv);
 #pragma unroll
@@ -355,7 +356,7 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
     }
 }
 
-template <int RECON, int NT>
+template <int RECON, int NT, bool SPLIT_HI>
 int launch_mixed(const stag_ctx *ctx, const MixedArgs &args, cudaStream_t st) {
     const Geom &g = ctx->g;
     int grid = ctx->num_sms;
@@ -368,7 +369,7 @@ int launch_mixed(const stag_ctx *ctx, const MixedArgs &args, cudaStream_t st) {
     if (fit > ctx->opt.cg_resident_slices) fit = ctx->opt.cg_resident_slices;
     a.res_r = fit >= 1; a.res_q = fit >= 2; a.res_p = fit >= 3;
     const size_t smem = slice * (size_t)(a.res_r + a.res_q + a.res_p);
-    auto kern = cg_mixed_kernel<RECON, NT>;
+    auto kern = cg_mixed_kernel<RECON, NT, SPLIT_HI>;
     STAG_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     STAG_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));

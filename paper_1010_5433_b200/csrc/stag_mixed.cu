@@ -237,7 +237,7 @@ static MixedLayout mixed_layout(const stag_ctx *ctx, int nshift) {
 // The inner stage as ONE persistent kernel with residual replacement (stag_cg_mixed_persist.cuh): fp32 matrices
 // and directions, fp64 solutions, true fp64 residual of the base system at every replacement.  Returns
 // STAG_ERR_UNSUPPORTED when that kernel does not apply (the caller then runs the plain fp32 stage).
-static int mixed_persistent(const stag_ctx *ctx, const void *packed_hi, const void *packed_lo, int recon,
+static int mixed_persistent(const stag_ctx *ctx, const void *packed_hi, int prec_hi, const void *packed_lo, int recon,
                             const void *b64, double mass, int nshift, const double *shifts, double stop,
                             int maxiter, void *x64, char *ws, const MixedLayout &lay, stag_cg_info *info,
                             int *replacements, cudaStream_t st) {
@@ -272,8 +272,13 @@ static int mixed_persistent(const stag_ctx *ctx, const void *packed_hi, const vo
     a.partials = reinterpret_cast<double *>(cw + cl.partials);
     a.ru_delta = 1.0 / (double)(ctx->opt.cg_mixed_delta_inv > 0 ? ctx->opt.cg_mixed_delta_inv : 10);
     const int nt = ctx->opt.cg_persistent_threads;
-    int rc = recon == 18 ? (nt == 512 ? launch_mixed<18, 512>(ctx, a, st) : launch_mixed<18, 1024>(ctx, a, st))
-                         : (nt == 512 ? launch_mixed<12, 512>(ctx, a, st) : launch_mixed<12, 1024>(ctx, a, st));
+    int rc;
+    if (prec_hi == STAG_F64_SPLIT)
+        rc = recon == 18 ? (nt == 512 ? launch_mixed<18, 512, true>(ctx, a, st) : launch_mixed<18, 1024, true>(ctx, a, st))
+                         : (nt == 512 ? launch_mixed<12, 512, true>(ctx, a, st) : launch_mixed<12, 1024, true>(ctx, a, st));
+    else
+        rc = recon == 18 ? (nt == 512 ? launch_mixed<18, 512, false>(ctx, a, st) : launch_mixed<18, 1024, false>(ctx, a, st))
+                         : (nt == 512 ? launch_mixed<12, 512, false>(ctx, a, st) : launch_mixed<12, 1024, false>(ctx, a, st));
     if (rc) { cudaGetLastError(); return rc; }
     STAG_CUDA_OK(cudaMemcpyAsync(h, cw + cl.state, sizeof(CgState), cudaMemcpyDeviceToHost, st));
     STAG_CUDA_OK(cudaStreamSynchronize(st));
@@ -369,8 +374,8 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     // (32^3 x 8: 0.107 s against 0.169 s in fp64; with more shifts the shifted systems stop at the fp32
     // rounding of the matrices times ||x_i||/||b|| and the polish costs as much as after the plain fp32 run) | 2 always
     const bool want_ru = ctx->opt.cg_mixed_reliable == 2 || (ctx->opt.cg_mixed_reliable == 1 && nshift == 1);
-    if (want_ru && ctx->opt.cg_persistent && prec_hi == STAG_F64 && recon_hi == recon_lo)
-        rc = mixed_persistent(ctx, packed_hi, packed_lo, recon_lo, b_even, mass, nshift, host_shifts, stop, maxiter,
+    if (want_ru && ctx->opt.cg_persistent && recon_hi == recon_lo)
+        rc = mixed_persistent(ctx, packed_hi, prec_hi, packed_lo, recon_lo, b_even, mass, nshift, host_shifts, stop, maxiter,
                               x_even, ws, lay, &mi.inner, &mi.reliable_updates, st);
     if (rc != STAG_ERR_UNSUPPORTED) {
         if (rc != STAG_OK && rc != STAG_ERR_NOTCONV) {

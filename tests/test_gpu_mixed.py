@@ -90,14 +90,14 @@ def test_polish_from_shared_start_matches_oracle_polish(stag, prec_name, recon, 
 @pytest.mark.parametrize("hi,recon_hi,recon_lo,reliable", [("F64", 18, 18, 2), ("F64", 12, 12, 2), ("F64", 18, 18, 1),
                                                            ("F64", 18, 12, 2), ("F64_SPLIT", 18, 18, 2)])
 def test_mixed_config1(stag, hi, recon_hi, recon_lo, reliable):
-    """reliable = 2 (forced; the default 1 uses it for single-shift solves only) with native fp64 matrices of the same recon: the inner stage is the persistent kernel with
+    """reliable = 2 (forced; the default 1 uses it for single-shift solves only) with fp64 or split-double matrices of the same recon: the inner stage is the persistent kernel with
     residual replacement (fp32 matrices, fp64 x_i, convergence on the TRUE fp64 residual of the base system);
-    otherwise (option off, split-double, different recon) the plain fp32 stage + polish."""
+    otherwise (option at its default with several shifts, different recon) the plain fp32 stage + polish."""
     cfg = si.get_config("c1_4x4x4x4")
     L, U, b, m, shifts = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"], cfg["shifts"]
     ctx = stag.Stag(L)
     ctx.set_option("cg_mixed_reliable", reliable)
-    replaced = reliable == 2 and hi == "F64" and recon_hi == recon_lo
+    replaced = reliable == 2 and recon_hi == recon_lo
     prec_hi = getattr(stag, hi)
     p_hi = ctx.upload_gauge(U, prec_hi, recon_hi)
     p_lo = p_hi if hi == "F64_SPLIT" else ctx.upload_gauge(U, stag.F32, recon_lo)   # N3: one buffer, both precisions
@@ -132,7 +132,8 @@ def test_mixed_config1(stag, hi, recon_hi, recon_lo, reliable):
 
 @pytest.mark.parametrize("slices", [3, 1, 0])
 @pytest.mark.parametrize("recon", [18, 12])
-def test_mixed_single_shift_residual_replacement(stag, slices, recon):
+@pytest.mark.parametrize("hi", ["F64", "F64_SPLIT"])
+def test_mixed_single_shift_residual_replacement(stag, slices, recon, hi):
     """Single shift, default options: the inner stage is the persistent residual-replacement kernel; it must stop
     on the TRUE residual (nothing left to polish), in about as many iterations as the fp64 oracle, in every
     shared-memory residency case."""
@@ -140,11 +141,13 @@ def test_mixed_single_shift_residual_replacement(stag, slices, recon):
     L, U, b, m, shifts = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"], cfg["shifts"]
     ctx = stag.Stag(L)
     ctx.set_option("cg_resident_slices", slices)
-    p64, p32 = ctx.upload_gauge(U, stag.F64, recon), ctx.upload_gauge(U, stag.F32, recon)
+    prec_hi = getattr(stag, hi)
+    p64 = ctx.upload_gauge(U, prec_hi, recon)
+    p32 = p64 if hi == "F64_SPLIT" else ctx.upload_gauge(U, stag.F32, recon)      # N3: one buffer, both precisions
     vb = ctx.vector_bytes(stag.F64)
     x, ws = ctx.alloc(vb), ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(1))
     x.fill_(0xFF)
-    rc, info = ctx.mshift_cg_mixed(p64, stag.F64, recon, p32, recon, ctx.upload_vector(b, stag.F64), m, shifts,
+    rc, info = ctx.mshift_cg_mixed(p64, prec_hi, recon, p32, recon, ctx.upload_vector(b, stag.F64), m, shifts,
                                    1e-10, 20000, x, ws)
     ref = oracle.mshift_cg(L, U, b, m, shifts, 1e-10, 20000)
     assert rc == 0 and info["inner"]["converged"] and info["inner"]["kernel_launches"] == 1, info
@@ -152,7 +155,7 @@ def test_mixed_single_shift_residual_replacement(stag, slices, recon):
     assert abs(info["inner"]["iters"] - ref["iters"]) <= max(3, ref["iters"] // 10)
     assert true_res(L, U, m, shifts[0], b, ctx.download_vector(x, stag.F64)) <= 1e-10
     # maxiter reached: reports NOTCONV with the true residual it got to
-    rc, info = ctx.mshift_cg_mixed(p64, stag.F64, recon, p32, recon, ctx.upload_vector(b, stag.F64), m, shifts,
+    rc, info = ctx.mshift_cg_mixed(p64, prec_hi, recon, p32, recon, ctx.upload_vector(b, stag.F64), m, shifts,
                                    1e-10, 5, x, ws)
     assert rc == stag.ERR_NOTCONV and info["inner"]["iters"] == 5 and info["polish"]["resid_after"][0] > 1e-10
 
