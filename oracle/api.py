@@ -14,6 +14,11 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "stag_oracle.cpp")
 _SO = os.path.join(_HERE, "libstag_oracle.so")
+# STAG_ORACLE_SANITIZE=1: the same source built with -fsanitize=address,undefined; the process
+# must then run with libasan preloaded (tests/test_oracle_sanitized.py does that in a subprocess).
+_SANITIZE = os.environ.get("STAG_ORACLE_SANITIZE") == "1"
+if _SANITIZE:
+    _SO = os.path.join(_HERE, "libstag_oracle_san.so")
 _lib = None
 
 
@@ -21,7 +26,11 @@ def build(force: bool = False) -> str:
     """Compile the oracle with g++ (building the checker is not using it)."""
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
         tmp = _SO + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["g++", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=c++14",
+        opt = ["-O2"]
+        if _SANITIZE:
+            opt = ["-O1", "-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined",
+                   "-fno-sanitize-recover=all"]
+        subprocess.check_call(["g++"] + opt + ["-fopenmp", "-fPIC", "-shared", "-std=c++14",
                                "-ffp-contract=off", "-o", tmp, _SRC])
         os.replace(tmp, _SO)
     return _SO

@@ -348,14 +348,13 @@ class Stag:
 
     # ---- conveniences for tests / bench: torch copies + the calls above, no arithmetic ----------
     def upload_gauge(self, links: np.ndarray, prec: int, recon: int, keep_canonical=None) -> torch.Tensor:
-        """host canonical links complex128 [V][4][3][3] -> packed device buffer."""
+        """host canonical links complex128 [V][4][3][3] -> packed device buffer.  keep_canonical: a caller-owned
+        device buffer of gauge_canonical_bytes() that receives the canonical copy (always re-loaded from `links`)."""
         links = np.ascontiguousarray(links, dtype=np.complex128)
         assert links.size == self.V * 36, links.shape
         canon = keep_canonical if keep_canonical is not None else self.alloc(self.gauge_canonical_bytes())
-        if keep_canonical is None or not getattr(self, "_canon_loaded", False):
-            self.gauge_load(links, canon)
-            torch.cuda.current_stream().synchronize()      # pageable source: do not return early
-            self._canon_loaded = keep_canonical is not None
+        self.gauge_load(links, canon)
+        torch.cuda.current_stream().synchronize()          # pageable source: do not return early
         packed = self.alloc(self.gauge_packed_bytes(prec, recon))
         self.gauge_pack(canon, packed, prec, recon)
         torch.cuda.current_stream().synchronize()

@@ -146,7 +146,7 @@ def test_c4_block_cg_four_sources(stag, c4):
     x1, ws1 = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(0, n))
     for s, b in enumerate(srcs):
         nb = np.linalg.norm(b)
-        for i in (0, 1, 5, 15):
+        for i in range(n):                                   # north_star: "for every shift"
             xi = ctx.download_vector(x, 0, (s * n + i) * vb)
             assert np.linalg.norm(b - oracle.apply_A(L, U, m, shifts[i], xi)) / nb <= stop, (s, i)
         rc1, info1 = ctx.mshift_cg(packed, 0, 18, ctx.upload_vector(b, 0), m, shifts, stop, 100000, x1, ws1)
@@ -180,6 +180,35 @@ def test_c4_multishift_cg_bench_configuration(stag, c4, path):
 test_c4_multishift_cg_bench_configuration.iters = {}
 
 
+@pytest.mark.parametrize("path", ["persistent", "multikernel"])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_c4_fp32_multishift_cg_reading_A9(stag, c4, path, recon):
+    """The solve `bench.py --prec f32` times (32^3x8, 16 shifts, fp32 vectors and links, fp64 reductions), reading
+    A9 / PAPER.md:127: stop 1e-10 is out of reach, so the run must end on stagnation (or stop), without breakdown,
+    with a TRUE residual of every shift — by the oracle's fp64 operator — below 1e-2 (the paper's "10^-2 - 10^-3"
+    floor for this conditioning) and an honest report of where it stopped."""
+    cfg, U, srcs = c4
+    L, b, shifts, m = cfg["L"], srcs[0], cfg["shifts"], cfg["mass"]
+    n = len(shifts)
+    ctx = stag.Stag(L)
+    ctx.set_option("cg_persistent", 1 if path == "persistent" else 0)
+    packed = ctx.upload_gauge(U, 1, recon)
+    vb = ctx.vector_bytes(1)
+    x, ws = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(1, n))
+    rc, info = ctx.mshift_cg(packed, 1, recon, ctx.upload_vector(b, 1), m, shifts, cfg["stops"][0], 100000, x, ws)
+    assert rc in (stag.OK, stag.ERR_NOTCONV) and not info["breakdown"]
+    assert info["converged"] or info["stagnated"]
+    assert (info["kernel_launches"] == 1) == (path == "persistent")
+    assert 1000 < info["iters"] < 6000, info["iters"]          # the fp64 solve needs 2988
+    nb = np.linalg.norm(b)
+    worst = 0.0
+    for i, s in enumerate(shifts):
+        xi = ctx.download_vector(x, 1, i * vb)
+        assert np.all(np.isfinite(xi))
+        worst = max(worst, np.linalg.norm(b - oracle.apply_A(L, U, m, s, xi)) / nb)
+    assert worst < 1e-2, worst
+
+
 def test_c4_iteration_count_matches_oracle(stag, c4, threads):
     """Iterations within +-2 of the oracle's own full solve (3000 iterations of the plain C++ CG)."""
     cfg, U, srcs = c4
@@ -197,6 +226,8 @@ def test_c5_dslash_fp64_and_fp32_full_compare(stag, threads):
     cfg = si.get_config("c5_64x64x64x64")
     L, U, v = cfg["L"], si.make_links(cfg), si.make_source(cfg)
     want = oracle.dslash_oe(L, U, v)
+    v_odd = si.source_gaussian(L, cfg["seed"], stream=7)          # an independent vector on the odd sites
+    want_eo = oracle.dslash_eo(L, U, v_odd)                       # D_eo reads the OTHER eight packed link sets
     ctx = stag.Stag(L)
     canon = ctx.alloc(ctx.gauge_canonical_bytes())
     ctx.gauge_load(U, canon)
@@ -206,12 +237,15 @@ def test_c5_dslash_fp64_and_fp32_full_compare(stag, threads):
         vin, w = ctx.upload_vector(v, prec), ctx.alloc(ctx.vector_bytes(prec))
         ctx.dslash_oe(packed, prec, recon, vin, w)
         assert rel(ctx.download_vector(w, prec), want) <= (1e-5 if prec == 1 else 1e-13), (prec, recon)
+        vin = ctx.upload_vector(v_odd, prec)
+        ctx.dslash_eo(packed, prec, recon, vin, w)
+        assert rel(ctx.download_vector(w, prec), want_eo) <= (1e-5 if prec == 1 else 1e-13), ("eo", prec, recon)
         del packed, vin, w
 
 
 def test_c5_multishift_cg_true_residuals(stag, threads):
     """Config 5 as bench.py --workload c5 runs it (64^4, 8 shifts, stop 1e-9, multi-kernel path replayed as CUDA
-    graphs): the TRUE residual of the lightest and the heaviest shift by the oracle's operator.  The oracle's own
+    graphs): the TRUE residual of EVERY shift by the oracle's operator.  The oracle's own
     solve at this size is hours on one core, so the iteration count is not compared."""
     cfg = si.get_config("c5_64x64x64x64")
     L, U, b, m, shifts, stop = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"], cfg["shifts"], cfg["stops"][0]
@@ -223,7 +257,7 @@ def test_c5_multishift_cg_true_residuals(stag, threads):
     assert rc == 0 and info["converged"] and info["kernel_launches"] > 1
     assert info["iters_shift"][0] == info["iters"] and info["iters_shift"][-1] < info["iters"]   # heavy shifts freeze early
     nb = np.linalg.norm(b)
-    for i in (0, n - 1):
+    for i in range(n):
         xi = ctx.download_vector(x, 0, i * vb)
         tr = np.linalg.norm(b - oracle.apply_A(L, U, m, shifts[i], xi)) / nb
         assert tr <= stop, (i, tr)
@@ -252,9 +286,9 @@ def test_paper_shape_4x48cubed_cg_and_dslash(stag, threads, path):
     assert rc == 0, info
     assert (info["kernel_launches"] == 1) == (path == "persistent")
     nb = np.linalg.norm(b)
-    for i in (0, 3, 7):
+    for i in range(n):
         xi = ctx.download_vector(x, 0, i * vb)
-        assert np.linalg.norm(b - oracle.apply_A(L, U, m, shifts[i], xi)) / nb <= stop
+        assert np.linalg.norm(b - oracle.apply_A(L, U, m, shifts[i], xi)) / nb <= stop, i
     test_paper_shape_4x48cubed_cg_and_dslash.iters = getattr(test_paper_shape_4x48cubed_cg_and_dslash, "iters", {})
     test_paper_shape_4x48cubed_cg_and_dslash.iters[path] = info["iters"]
     it = test_paper_shape_4x48cubed_cg_and_dslash.iters
