@@ -320,7 +320,8 @@ static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, 
     bool persistent = ctx->opt.cg_persistent != 0 && cg_persistent_fits(ctx, prec);
     if (persistent) {
         // small lattice: the whole solve is one cooperative launch (stag_cg_persist.cu)
-        const int prc = cg_persistent_dispatch(ctx, packed, prec, recon, b, x, L.x_stride, y, L.ws, L.lay, st);
+        const int prc = cg_persistent_dispatch(ctx, packed, prec, recon, b, nshift, shifts, x, L.x_stride, y, L.ws,
+                                               L.lay, st);
         if (prc == STAG_ERR_UNSUPPORTED) persistent = false;       // cannot be co-resident: multi-kernel path
         else if (prc) { cudaGetLastError(); return prc; }
         else launches = 1;

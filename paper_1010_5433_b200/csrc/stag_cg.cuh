@@ -34,8 +34,10 @@ struct CgState {
     unsigned int ticket;    // last-block detection for the grid-wide reductions
 };
 
+static constexpr size_t kPersistFlagBytes = 256 * 128;   // kMaxPersistGrid CTAs (stag_cg_persist.cuh)
+
 struct CgLayout {
-    size_t state, partials, r, q, w, p;   // byte offsets into the workspace; p = nshift vectors
+    size_t state, partials, flags, r, q, w, p;   // byte offsets into the workspace; p = nshift vectors
     size_t vec_stride;                    // bytes between consecutive p_i
     int max_grid;                         // doubles reserved at `partials`
 };
@@ -53,6 +55,7 @@ inline size_t cg_workspace_layout(const stag_ctx *ctx, int prec, int nshift, CgL
     l.state = off;    off += align256(sizeof(CgState));
     l.max_grid = cg_max_grid(ctx);
     l.partials = off; off += align256(sizeof(double) * (size_t)l.max_grid);
+    l.flags = off;    off += kPersistFlagBytes;      // persistent kernel: one epoch word per CTA and 128-byte line
     l.r = off;        off += vec;
     l.q = off;        off += vec;
     l.w = off;        off += vec;
@@ -146,7 +149,7 @@ int block_solve(const stag_ctx *ctx, const void *packed, int prec, int recon, in
 // implemented in stag_cg_persist.cu: the whole solve as one cooperative kernel (small lattices)
 bool cg_persistent_fits(const stag_ctx *ctx, int prec);
 int cg_persistent_dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon,
-                           const void *b, void *x, size_t x_stride, void *y, char *ws,
-                           const CgLayout &lay, cudaStream_t st);
+                           const void *b, int nshift, const double *host_shifts, void *x, size_t x_stride,
+                           void *y, char *ws, const CgLayout &lay, cudaStream_t st);
 
 }  // namespace stag

@@ -14,13 +14,13 @@ STAG_DEFINE_PERSIST_R(1)
 // iteration takes milliseconds, launch ramps and reduction tails no longer matter, and the multi-kernel path
 // (which runs at the copy bandwidth at 64^4) is used.
 bool cg_persistent_fits(const stag_ctx *ctx, int prec) {
-    const int S = sites_per_cta(ctx->g.Vh, ctx->num_sms);
-    return (size_t)2 * S * vec_bytes_per_site(prec) <= kMaxDynSmem;
+    if (persist_grid(ctx) > kMaxPersistGrid) return false;
+    return (size_t)2 * persist_slots(ctx) * vec_bytes_per_site(prec) <= kMaxDynSmem;
 }
 
 int cg_persistent_dispatch(const stag_ctx *ctx, const void *packed, int prec, int recon,
-                           const void *b, void *x, size_t x_stride, void *y, char *ws,
-                           const CgLayout &lay, cudaStream_t st) {
+                           const void *b, int nshift, const double *host_shifts, void *x, size_t x_stride,
+                           void *y, char *ws, const CgLayout &lay, cudaStream_t st) {
     PersistArgs a;
     std::memset(&a, 0, sizeof(a));
     a.W = static_cast<const char *>(packed);
@@ -38,14 +38,16 @@ int cg_persistent_dispatch(const stag_ctx *ctx, const void *packed, int prec, in
     a.state = reinterpret_cast<CgState *>(ws + lay.state);
     a.state_stride = align256(sizeof(CgState));
     a.partials = reinterpret_cast<double *>(ws + lay.partials);
+    a.flags = reinterpret_cast<unsigned int *>(ws + lay.flags);
     a.nrhs = 1;
+    a.keep_mask = persist_keep_mask(ctx, prec, 1, nshift, host_shifts);
     if (prec == STAG_F64_SPLIT) return cg_persistent_launch_split(ctx, recon, 1, a, st);
     return cg_persistent_launch_r<1>(ctx, prec, recon, a, st);
 }
 
 // ---- block solve -----------------------------------------------------------------------------------
 struct BlockLayout {
-    size_t state, partials, r, q, w, p, total;
+    size_t state, partials, flags, r, q, w, p, total;
     size_t vec_stride, state_stride;
 };
 
@@ -56,6 +58,7 @@ static BlockLayout block_layout(const stag_ctx *ctx, int prec, int nshift, int n
     l.state_stride = align256(sizeof(CgState));
     l.state = off;    off += l.state_stride * (size_t)nrhs;
     l.partials = off; off += align256(sizeof(double) * 2 * STAG_MAX_RHS * (size_t)ctx->num_sms);
+    l.flags = off;    off += kPersistFlagBytes;
     l.r = off;        off += vec * (size_t)nrhs;
     l.q = off;        off += vec * (size_t)nrhs;
     l.w = off;        off += vec * (size_t)nrhs;
@@ -150,7 +153,10 @@ int stag::block_solve(const stag_ctx *ctx, const void *packed, int prec, int rec
     a.state = reinterpret_cast<CgState *>(ws + lay.state);
     a.state_stride = lay.state_stride;
     a.partials = reinterpret_cast<double *>(ws + lay.partials);
+    a.flags = reinterpret_cast<unsigned int *>(ws + lay.flags);
     a.nrhs = nrhs;
+    // N2 polish (one shift per source): every e_s is live to the end and small enough to stay in L2
+    a.keep_mask = persist_keep_mask(ctx, prec, nrhs, nshift, host_shifts);
     int rc = prec == STAG_F64_SPLIT ? cg_persistent_launch_split(ctx, recon, nrhs == 1 ? 1 : nrhs == 2 ? 2 : 4, a, st)
            : nrhs == 1 ? cg_persistent_launch_r<1>(ctx, prec, recon, a, st)
            : nrhs == 2 ? cg_persistent_launch_r<2>(ctx, prec, recon, a, st)

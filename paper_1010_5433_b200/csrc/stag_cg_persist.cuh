@@ -14,10 +14,16 @@
 //   phase C  every CTA adds the partials in the same order (bit-identical alpha everywhere),
 //            runs the a4 recurrences in its own shared memory, then r -= alpha q with r and q
 //            both in shared memory (a5 moves no HBM bytes at all); partial of <r,r>; grid barrier
-//   phase D  every CTA: beta, beta_i, zeta_i, convergence latch, freezing (a4, a7); then a6:
-//            the base shift first (p_base is what the neighbours need), ARRIVE at the barrier,
-//            the other live shifts' x_i, p_i streamed once, then WAIT — the barrier latency hides
-//            behind the shift updates.
+//   phase D  every CTA: beta, beta_i, zeta_i, convergence latch, freezing (a4, a7); then the base shift of a6
+//            (p_base is what the neighbours gather next).  The other live shifts' x_i, p_i updates are DEFERRED:
+//            they are worked off, one CTA-wide pass at a time, while the CTA waits at the sync points of the
+//            next iteration (a wait is skew + barrier latency during which HBM would idle), and whatever is left
+//            is forced before phase D overwrites their coefficients.  r and q swap buffers every iteration so
+//            that the old r stays readable until then.
+//   sync     after B and C: grid-wide (the two reductions).  After A and D a CTA needs w / p_base only from the
+//            CTAs that own its neighbouring sites: per-CTA epoch flags instead of a grid barrier.
+//   L2       x_i, p_i of the lightest shifts (the longest-lived) are marked evict_last, the hopping matrices
+//            evict_first: what fits of the shift vectors stays in the 126 MB L2 across iterations.
 //
 // r, q and the CTA's own slice of p_base live in shared memory for the whole solve when they fit
 // (3 x 48 B x sites/SM x R: 129 KB at 32^3 x 8, R = 1); what does not fit (priority r, q, p) stays
@@ -37,8 +43,9 @@
 
 // Per-phase timers (build with -DSTAG_PHASE_TIMERS: `STAG_PHASE_TIMERS=1 python -m paper_1010_5433_b200._build`
 // writes libstag_b200_timers.so, which the binding loads when the same variable is set).  CTAs 0, 77 and the last
-// one print, at the end of the solve, the mean microseconds per iteration they spent in each phase and in each
-// grid-barrier wait (%globaltimer, CTA-wide: a __syncthreads precedes every tick).  Compiles to nothing otherwise.
+// one print, at the end of the solve, the mean microseconds per iteration they spent in each phase, at each sync
+// point (arrive + deferred shift updates worked off while waiting + wait) and in the shift updates that had to be
+// forced before phase D (%globaltimer, CTA-wide: a __syncthreads precedes every tick).  Compiles to nothing otherwise.
 #ifdef STAG_PHASE_TIMERS
 #include <cstdio>
 #define STAG_T_DECL                                                                       \
@@ -52,12 +59,15 @@
         t0_ = t1_;                                                                        \
     } while (0)
 #define STAG_T_REPORT(R_, iters_)                                                                          \
-    if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == gridDim.x - 1)) {       \
+    if (threadIdx.x == 0 && (blockIdx.x == 0 || blockIdx.x == 77 || blockIdx.x == gridDim.x - 1 ||         \
+                             STAG_PHASE_TIMERS > 1)) {                                                     \
         const double k_ = 1e-3 / ((iters_) > 0 ? (iters_) : 1);                                            \
-        printf("[stag timers] CTA %d R=%d iters %d  us/iter: A %.2f wait %.2f | B %.2f wait %.2f | C %.2f " \
-               "wait %.2f | D base %.2f shifts %.2f wait %.2f\n", (int)blockIdx.x, R_, (int)(iters_),      \
+        unsigned smid_;                                                                                    \
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid_));                                                 \
+        printf("[stag timers] CTA %d sm %u R=%d iters %d  us/iter: A %.2f sync %.2f | B %.2f sync %.2f | C %.2f " \
+               "sync %.2f | D %.2f sync %.2f\n", (int)blockIdx.x, smid_, R_, (int)(iters_),                 \
                tt_[0] * k_, tt_[1] * k_, tt_[2] * k_, tt_[3] * k_, tt_[4] * k_, tt_[5] * k_, tt_[6] * k_,  \
-               tt_[7] * k_, tt_[8] * k_);                                                                  \
+               tt_[7] * k_);                                                                               \
     }
 #else
 #define STAG_T_DECL
@@ -133,7 +143,49 @@ struct Slice {
     }
 };
 
-// ---- streaming (evict-first) own-site access to x_i, p_i -----------------------------------------
+// ---- own-site access to x_i, p_i with an explicit L2 eviction policy -------------------------------
+// Every x_i, p_i element is read and written by exactly one thread, once per iteration: L1 is bypassed.  In L2
+// the vectors of the KEEP set (the lightest shifts, which stay live longest; PersistArgs::keep_mask) are marked
+// evict_last so that they survive the 2 x 151 MB of hopping matrices (evict_first) that stream through the
+// 126 MB L2 every iteration: their 192 B per site and iteration then never reach HBM.  All other shifts stream
+// (evict_first).
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t pol;
+    asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+__device__ __forceinline__ void load_vec_pol(const char *v, int Vh, int e, double (&x)[6], uint64_t pol) {
+    const double2 *p = reinterpret_cast<const double2 *>(v) + e;
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;"
+                     : "=d"(x[2 * c]), "=d"(x[2 * c + 1]) : "l"(p + (size_t)c * Vh), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void load_vec_pol(const char *v, int Vh, int e, float (&x)[6], uint64_t pol) {
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=f"(x[0]), "=f"(x[1]), "=f"(x[2]), "=f"(x[3])
+                 : "l"(reinterpret_cast<const float4 *>(v) + e), "l"(pol) : "memory");
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;"
+                 : "=f"(x[4]), "=f"(x[5])
+                 : "l"(reinterpret_cast<const float2 *>(v + (size_t)Vh * 16) + e), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void store_vec_pol(char *v, int Vh, int e, const double (&x)[6], uint64_t pol) {
+    double2 *p = reinterpret_cast<double2 *>(v) + e;
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;"
+                     :: "l"(p + (size_t)c * Vh), "d"(x[2 * c]), "d"(x[2 * c + 1]), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void store_vec_pol(char *v, int Vh, int e, const float (&x)[6], uint64_t pol) {
+    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;"
+                 :: "l"(reinterpret_cast<float4 *>(v) + e), "f"(x[0]), "f"(x[1]), "f"(x[2]), "f"(x[3]), "l"(pol)
+                 : "memory");
+    asm volatile("st.global.L1::no_allocate.L2::cache_hint.v2.f32 [%0], {%1,%2}, %3;"
+                 :: "l"(reinterpret_cast<float2 *>(v + (size_t)Vh * 16) + e), "f"(x[4]), "f"(x[5]), "l"(pol)
+                 : "memory");
+}
+
+// ---- streaming (evict-first) own-site access, used by the mixed-precision kernel ---------------------
 __device__ __forceinline__ void load_vec_cs(const char *v, int Vh, int e, double (&x)[6]) {
     const double2 *p = reinterpret_cast<const double2 *>(v) + e;
 #pragma unroll
@@ -243,11 +295,22 @@ struct PersistArgs {
     char *y;              // nullable; R vectors, stride x_stride
     CgState *state;       // R states, stride state_stride bytes
     size_t state_stride;
-    double *partials;     // 2 * R * gridDim.x doubles
-    int S;                // sites per CTA (multiple of 32)
+    double *partials;     // 2 * R * gridDim.x doubles: per-CTA partials of <p,q>, then of <r,r>
+    unsigned int *flags;  // gridDim.x epoch words, one per 128-byte line (zeroed by the host before the launch)
+    int S;                // slots per CTA and source in a resident slice = the largest CTA's sites (multiple of 32)
     int nrhs;             // sources actually present (<= R)
     int res_r, res_q, res_p;   // which slices are resident in shared memory
+    unsigned keep_mask;   // shifts whose x_i, p_i are kept L2-resident (evict_last); the others stream
+    int fill;             // 1: deferred shift updates are worked off while the CTA waits at a sync point
+    int nbflags;          // 1: phases A->B and D->A wait for the owners of the neighbouring sites only; 0: for every CTA
 };
+
+// The CTA's contiguous range of 32-site tiles: tiles [c T / G, (c+1) T / G) of T, so the sizes differ by at most
+// one tile and no SM idles (32^3 x 8 on 148 SMs: 100 CTAs of 28 tiles, 48 of 27).
+__host__ __device__ __forceinline__ int cta_first_tile(int c, int T, int G) { return (int)((long long)c * T / G); }
+__device__ __forceinline__ int tile_owner(int t, int T, int G) { return (int)((((long long)t + 1) * G - 1) / T); }
+
+static constexpr int kMaxPersistGrid = 256;          // CTAs (= SMs) the neighbour tables are sized for
 
 template <typename T, int RECON, int NT, int R, bool SPLIT = false>
 __global__ void __launch_bounds__(NT, 1)
@@ -256,13 +319,18 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
     __shared__ Scalars<T> sc[R];
     __shared__ double red[(NT / 32) * R];
     __shared__ int n_running;
+    __shared__ unsigned int nb_mask[kMaxPersistGrid / 32];
+    __shared__ int nb_list[kMaxPersistGrid];
+    __shared__ int nb_n;
+    __shared__ unsigned int sync_seen;               // number of the last sync point warp 0 has seen released
 
     constexpr int LS = NT / R;                       // streaming phases: sites per pass and source
     const int tid = threadIdx.x, G = gridDim.x, Vh = g.Vh, S = a.S;
     const int rhs = tid / LS, l0 = tid % LS;         // streaming phases: this thread's source (warp-uniform)
-    const int e0 = min(Vh, (int)blockIdx.x * S), ns = min(Vh, e0 + S) - e0;
+    const int tiles = (Vh + 31) >> 5;
+    const int e0 = min(Vh, cta_first_tile(blockIdx.x, tiles, G) << 5);
+    const int ns = min(Vh, cta_first_tile(blockIdx.x + 1, tiles, G) << 5) - e0;
     unsigned int *bar = &a.state->ticket;
-    unsigned int epoch = 0;
     double *part_pq = a.partials, *part_rr = a.partials + (size_t)R * G;
 
     CgState *st = reinterpret_cast<CgState *>(reinterpret_cast<char *>(a.state) + (size_t)rhs * a.state_stride);
@@ -276,7 +344,12 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
     char *x_base = x_r + (size_t)base * a.x_stride;
     const size_t pb_stride = (size_t)nshift * a.p_stride;       // between the sources' p_base
     char *p_base0 = a.p + (size_t)base * a.p_stride;            // p_base of source 0
+    // L2 policy of shift i's x_i, p_i (made where it is used: two registers less across the stencil phases)
+    auto shift_policy = [&](int i) { return ((a.keep_mask >> i) & 1u) ? policy_evict_last() : policy_evict_first(); };
 
+    // r and q swap roles every iteration when both live in the same kind of memory: phase C then writes the new
+    // r over q and leaves the old r intact for the deferred shift updates still pending (see the sync point)
+    const bool swap_rq = a.res_r == a.res_q;
     Slice<T> r_s, q_s, p_s;
     {
         const size_t slice = (size_t)S * R * 6 * sizeof(T);
@@ -289,6 +362,34 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
         if (p_s.res) { p_s.s.init(d, S * R); d += slice; }
     }
     const bool present = rhs < a.nrhs;
+
+    // ---- the CTAs that own a neighbour of one of this CTA's sites (either parity) ---------------------
+    if (tid < kMaxPersistGrid / 32) nb_mask[tid] = 0u;
+    if (tid == 0) { nb_n = 0; sync_seen = 0u; }
+    __syncthreads();
+    if (a.nbflags) {
+        for (int ls = tid; ls < 2 * ns; ls += NT) {
+            const int par = ls >= ns, e = e0 + (par ? ls - ns : ls);
+            const Site s = site_of(g, e, par);
+            const int x[4] = {s.x0, s.x1, s.x2, s.x3};
+            int stride = 1;
+#pragma unroll
+            for (int mu = 0; mu < 4; ++mu) {
+                const int Lmu = g.L[mu];
+                const int ef = (s.lex + stride - (x[mu] == Lmu - 1 ? Lmu * stride : 0)) >> 1;
+                const int eb = (s.lex - stride + (x[mu] == 0 ? Lmu * stride : 0)) >> 1;
+                const int of = tile_owner(ef >> 5, tiles, G), ob = tile_owner(eb >> 5, tiles, G);
+                if (of != (int)blockIdx.x) atomicOr(&nb_mask[of >> 5], 1u << (of & 31));
+                if (ob != (int)blockIdx.x) atomicOr(&nb_mask[ob >> 5], 1u << (ob & 31));
+                stride *= Lmu;
+            }
+        }
+        __syncthreads();
+    }
+    for (int c = tid; c < G; c += NT)
+        if (c != (int)blockIdx.x && (!a.nbflags || ((nb_mask[c >> 5] >> (c & 31)) & 1u))) nb_list[atomicAdd(&nb_n, 1)] = c;
+    __syncthreads();
+    const int nnb = nb_n;
 
     // ---- start: x_i = 0, r = p_i = b, bb = <b,b> ---------------------------------------------------
     if (tid < 32 * R && (tid & 31) < STAG_MAX_SHIFTS) {
@@ -313,15 +414,16 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                 r_s.store(slot, rhs, Vh, e, v);
                 if (p_s.res) p_s.s.store(slot, v);
                 for (int i = 0; i < nshift; ++i) {
+                    const uint64_t pol = shift_policy(i);
                     if (i == base) store_vec(p_base, Vh, e, v);
-                    else store_vec_cs(p_r + (size_t)i * a.p_stride, Vh, e, v);
-                    store_vec_cs(x_r + (size_t)i * a.x_stride, Vh, e, z);
+                    else store_vec_pol(p_r + (size_t)i * a.p_stride, Vh, e, v, pol);
+                    store_vec_pol(x_r + (size_t)i * a.x_stride, Vh, e, z, pol);
                 }
             }
         cta_partials_stream<NT, R>(acc, red, part_rr + blockIdx.x, G);
     }
-    grid_arrive(bar);
-    grid_wait(bar, ++epoch * G);
+    grid_arrive(bar);                                  // grid-wide: bb, and every p_base is in place for phase A
+    grid_wait(bar, (unsigned)G);
     if (tid < 32 * R) {
         const int s = tid >> 5;
         const double bb = grid_total(part_rr + (size_t)s * G, G);
@@ -357,29 +459,39 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
         wout[r] = a.w + (size_t)r * a.vec_stride;
     }
 
-    // ---- iterations -----------------------------------------------------------------------------------
+    // ---- iterations: a four-phase state machine around ONE sync point -----------------------------------
+    // (one copy of the sync-and-work-off code keeps the kernel inside its register budget: as a lambda called
+    // from four places it was not inlined and every captured variable went to local memory.  The stencil's
+    // instruction schedule — how many of a site's 96 loads are in flight — is sensitive to every register the
+    // surrounding code keeps alive across it: with two shifts per item instead of one the same stencil ran at 31
+    // instead of 23 us per phase.  profiles/README.md has the variants that were measured.)
+    //
+    // Deferred shift update (a6 of the iteration just finished), worked off in items: one item = one pass of
+    // the CTA over its sites (one site per thread) x one live shift.  Its state is in registers, identical in
+    // all threads of a source; the coefficients stay in sc[rhs] until phase D of the next iteration.  The r they
+    // need is r_s at every sync point: phase C leaves it alone (swap) and the roles only flip in phase D.
+    int pn = 0, pj = 0, ppass = 0, pnpass = 0;        // live shifts, next shift, next pass, passes (0: nothing pending)
+    bool act = false, act2 = false;
+    unsigned mask = 0;
+    unsigned int gepoch = 1, nepoch = 0;              // grid-wide barriers / neighbour syncs so far
+    int phase = 0;                                    // 0 A | 1 B | 2 C | 3 D
     STAG_T_DECL
-    while (n_running > 0) {
-        const bool act = sc[rhs].done == 0;          // streaming phases: this thread's source is still iterating
-        unsigned mask = 0;                           // stencil phases: the sources still iterating
+    while (n_running > 0 || phase != 0) {
+        if (phase == 0) {
+            act = sc[rhs].done == 0;                 // streaming phases: this thread's source is still iterating
+            mask = 0;                                // stencil phases: the sources still iterating
 #pragma unroll
-        for (int r = 0; r < R; ++r) mask |= (sc[r].done == 0 ? 1u : 0u) << r;
-
-        // phase A (a2): w = D_oe p_base on this CTA's odd sites
-        for (int ls = tid; ls < ns; ls += NT) {
-            T acc[R][6];
-            dslash_site_multi<T, RECON, R, false, SPLIT>(g, a.W, pin, mask, 1, e0 + ls, acc);
+            for (int r = 0; r < R; ++r) mask |= (sc[r].done == 0 ? 1u : 0u) << r;
+            // phase A (a2): w = D_oe p_base on this CTA's odd sites
+            for (int ls = tid; ls < ns; ls += NT) {
+                T acc[R][6];
+                dslash_site_multi<T, RECON, R, false, SPLIT>(g, a.W, pin, mask, 1, e0 + ls, acc);
 #pragma unroll
-            for (int r = 0; r < R; ++r)
-                if (R == 1 || ((mask >> r) & 1u)) store_vec(wout[r], Vh, e0 + ls, acc[r]);
-        }
-        STAG_TICK(0);
-        grid_arrive(bar);
-        grid_wait(bar, ++epoch * G);
-        STAG_TICK(1);
-
-        // phase B (a3): q = c0 p - D_eo w, partial Re<p,q>
-        {
+                for (int r = 0; r < R; ++r)
+                    if (R == 1 || ((mask >> r) & 1u)) store_vec(wout[r], Vh, e0 + ls, acc[r]);
+            }
+        } else if (phase == 1) {
+            // phase B (a3): q = c0 p - D_eo w, partial Re<p,q>
             double dot[R];
             T c0[R];
 #pragma unroll
@@ -402,35 +514,26 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                     }
             }
             cta_partials_all<NT, R>(dot, red, part_pq + blockIdx.x, G);
-        }
-        STAG_TICK(2);
-        grid_arrive(bar);
-        grid_wait(bar, ++epoch * G);
-        STAG_TICK(3);
-
-        // phase C (a4 after <p,q>, then a5): alpha, theta_new_i;  r -= alpha q;  partial <r,r>
-        if (tid < 32 * R) {
-            const int s = tid >> 5, i = tid & 31;
-            Scalars<T> &c = sc[s];
-            if (c.done == 0) {
-                const double pq = grid_total(part_pq + (size_t)s * G, G);
-                const double alpha = c.rr / pq;
-                const bool bad = !(pq > 0.0) || !isfinite(alpha);
-                const double k = alpha * c.beta_old / c.alpha_old;
-                __syncwarp();
-                if (!bad && i < nshift) {
-                    if (c.active[i] == 2) c.active[i] = 0;            // frozen at the previous iteration
-                    c.theta_new[i] = 1.0 / ((1.0 + c.delta[i] * alpha) + k * (1.0 - c.theta[i]));
-                }
-                if (i == 0) {
-                    c.pq = pq;
-                    if (bad) { c.breakdown = 1; c.done = 2; } else c.alpha = alpha;   // breakdown: no update
+        } else if (phase == 2) {
+            // phase C (a4 after <p,q>, then a5): alpha, theta_new_i;  r_new = r - alpha q;  partial <r,r>
+            if (tid < 32 * R) {
+                const int s = tid >> 5, i = tid & 31;
+                Scalars<T> &c = sc[s];
+                if (c.done == 0) {
+                    const double pq = grid_total(part_pq + (size_t)s * G, G);
+                    const double alpha = c.rr / pq;
+                    const bool bad = !(pq > 0.0) || !isfinite(alpha);
+                    const double k = alpha * c.beta_old / c.alpha_old;
+                    __syncwarp();
+                    if (!bad && i < nshift) c.theta_new[i] = 1.0 / ((1.0 + c.delta[i] * alpha) + k * (1.0 - c.theta[i]));
+                    if (i == 0) {
+                        c.pq = pq;
+                        if (bad) { c.breakdown = 1; c.done = 2; } else c.alpha = alpha;   // breakdown: no update
+                    }
                 }
             }
-        }
-        __syncthreads();
-        const bool act2 = act && sc[rhs].done == 0;
-        {
+            __syncthreads();
+            act2 = act && sc[rhs].done == 0;
             double acc = 0.0;
             if (act2) {
                 const T na = (T)(-sc[rhs].alpha);
@@ -444,128 +547,183 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                         rv[k] = fma(na, qv[k], rv[k]);
                         acc += (double)rv[k] * (double)rv[k];
                     }
-                    r_s.store(slot, rhs, Vh, e, rv);
+                    // with the swap the new r goes where q was and the old r stays readable for the pending items
+                    if (swap_rq) q_s.store(slot, rhs, Vh, e, rv); else r_s.store(slot, rhs, Vh, e, rv);
                 }
             }
             cta_partials_stream<NT, R>(acc, red, part_rr + blockIdx.x, G);
-        }
-        STAG_TICK(4);
-        grid_arrive(bar);
-        grid_wait(bar, ++epoch * G);
-        STAG_TICK(5);
-
-        // phase D (a4 after <r,r>, a7 latch, a6)
-        if (tid < 32 * R) {
-            const int s = tid >> 5, i = tid & 31;
-            Scalars<T> &c = sc[s];
-            if (c.done == 0) {
-                const double rr_new = grid_total(part_rr + (size_t)s * G, G);
-                const double alpha = c.alpha;
-                const double beta = rr_new / c.rr;
-                const double rel = sqrt(rr_new / c.bb);
-                const int iter = c.iter + 1;
-                bool live = false;
-                double th = 1.0, z = 1.0;
-                __syncwarp();
-                if (i < nshift) {
-                    th = c.theta_new[i];
-                    z = c.zeta[i] * th;
-                    c.zeta[i] = z;
-                    c.theta[i] = th;
-                    if (c.active[i] != 0) {
-                        live = true;
-                        if (c.active[i] == 1) {
+        } else {
+            // phase D (a4 after <r,r>, a7 latch, a6).  Nothing is pending here: the sync point before forced it.
+            if (tid < 32 * R) {
+                const int s = tid >> 5, i = tid & 31;
+                Scalars<T> &c = sc[s];
+                if (c.done == 0) {
+                    const double rr_new = grid_total(part_rr + (size_t)s * G, G);
+                    const double alpha = c.alpha;
+                    const double beta = rr_new / c.rr;
+                    const double rel = sqrt(rr_new / c.bb);
+                    const int iter = c.iter + 1;
+                    bool live = false;
+                    double th = 1.0, z = 1.0;
+                    __syncwarp();
+                    if (i < nshift) {
+                        if (c.active[i] == 2) c.active[i] = 0;            // frozen at the previous iteration
+                        th = c.theta_new[i];
+                        z = c.zeta[i] * th;
+                        c.zeta[i] = z;
+                        c.theta[i] = th;
+                        if (c.active[i] != 0) {
+                            live = true;
                             c.resid[i] = z * rel;
                             c.iters_shift[i] = iter;
                             if (freeze && i != base && z * rel <= 0.1 * c.stop) c.active[i] = 2;
                         }
                     }
-                }
-                const unsigned m = __ballot_sync(0xffffffffu, live && i != base);
-                if (live && i != base) {
-                    const int j = __popc(m & ((1u << i) - 1u));
-                    c.live[j] = i;
-                    c.ca[j] = (T)(alpha * th);
-                    c.cz[j] = (T)z;
-                    c.cb[j] = (T)(beta * th * th);
-                }
-                if (i == base) { c.a_base = (T)(alpha * th); c.z_base = (T)z; c.b_base = (T)(beta * th * th); }
-                if (i == 0) {
-                    c.nlive = __popc(m);
-                    c.alpha_old = alpha;
-                    c.beta_old = beta;
-                    c.rr = rr_new;
-                    c.iter = iter;
-                    int done = 0;
-                    if (rel <= c.stop) { c.converged = 1; done = 1; }
-                    else if (iter >= maxiter) done = 1;
-                    else if (!(rr_new == rr_new)) { c.breakdown = 1; done = 1; }
-                    else if (fp32) {                                     // reading A9
-                        if (rr_new < c.best_rr) { c.best_rr = rr_new; c.since_best = 0; }
-                        else if (++c.since_best >= 50) { c.stagnated = 1; done = 1; }
+                    const unsigned m = __ballot_sync(0xffffffffu, live && i != base);
+                    if (live && i != base) {
+                        const int j = __popc(m & ((1u << i) - 1u));
+                        c.live[j] = i;
+                        c.ca[j] = (T)(alpha * th);
+                        c.cz[j] = (T)z;
+                        c.cb[j] = (T)(beta * th * th);
                     }
-                    c.done = done;
+                    if (i == base) { c.a_base = (T)(alpha * th); c.z_base = (T)z; c.b_base = (T)(beta * th * th); }
+                    if (i == 0) {
+                        c.nlive = __popc(m);
+                        c.alpha_old = alpha;
+                        c.beta_old = beta;
+                        c.rr = rr_new;
+                        c.iter = iter;
+                        int done = 0;
+                        if (rel <= c.stop) { c.converged = 1; done = 1; }
+                        else if (iter >= maxiter) done = 1;
+                        else if (!(rr_new == rr_new)) { c.breakdown = 1; done = 1; }
+                        else if (fp32) {                                     // reading A9
+                            if (rr_new < c.best_rr) { c.best_rr = rr_new; c.since_best = 0; }
+                            else if (++c.since_best >= 50) { c.stagnated = 1; done = 1; }
+                        }
+                        c.done = done;
+                    }
                 }
             }
-        }
-        __syncthreads();
-        if (act2) {   // base shift first: its new p is what phase A of the next iteration gathers
-            const T ab = sc[rhs].a_base, zb = sc[rhs].z_base, bb_ = sc[rhs].b_base;
-            for (int ls = l0; ls < ns; ls += LS) {
-                const int e = e0 + ls, slot = rhs * S + ls;
-                T rv[6], pv[6], xv[6];
-                load_vec_cs(x_base, Vh, e, xv);
-                r_s.load(slot, rhs, Vh, e, rv);
-                p_s.load(slot, rhs, Vh, e, pv);
-#pragma unroll
-                for (int k = 0; k < 6; ++k) {
-                    xv[k] = fma(ab, pv[k], xv[k]);
-                    pv[k] = fma(zb, rv[k], bb_ * pv[k]);
-                }
-                store_vec_cs(x_base, Vh, e, xv);
-                if (p_s.res) p_s.s.store(slot, pv);
-                store_vec(p_base, Vh, e, pv);
-            }
-        }
-        STAG_TICK(6);
-        grid_arrive(bar);
-        if (act2) {
-            const Scalars<T> &c = sc[rhs];
-            const int n = c.nlive;
-            for (int ls = l0; ls < ns; ls += LS) {
-                const int e = e0 + ls, slot = rhs * S + ls;
-                T rv[6];
-                r_s.load(slot, rhs, Vh, e, rv);
-#pragma unroll 2
-                for (int j = 0; j < n; ++j) {
-                    char *xp = x_r + (size_t)c.live[j] * a.x_stride;
-                    char *pp = p_r + (size_t)c.live[j] * a.p_stride;
-                    const T aj = c.ca[j], zj = c.cz[j], bj = c.cb[j];
-                    T pv[6], xv[6];
-                    load_vec_cs(pp, Vh, e, pv);
-                    load_vec_cs(xp, Vh, e, xv);
+            __syncthreads();
+            if (swap_rq) { const Slice<T> t = r_s; r_s = q_s; q_s = t; }       // the new r is where q was
+            if (act2) {   // base shift first: its new p is what phase A of the next iteration gathers
+                const T ab = sc[rhs].a_base, zb = sc[rhs].z_base, bb_ = sc[rhs].b_base;
+                const uint64_t pol_base = shift_policy(base);
+                for (int ls = l0; ls < ns; ls += LS) {
+                    const int e = e0 + ls, slot = rhs * S + ls;
+                    T rv[6], pv[6], xv[6];
+                    load_vec_pol(x_base, Vh, e, xv, pol_base);
+                    r_s.load(slot, rhs, Vh, e, rv);
+                    p_s.load(slot, rhs, Vh, e, pv);
 #pragma unroll
                     for (int k = 0; k < 6; ++k) {
-                        xv[k] = fma(aj, pv[k], xv[k]);
-                        pv[k] = fma(zj, rv[k], bj * pv[k]);
+                        xv[k] = fma(ab, pv[k], xv[k]);
+                        pv[k] = fma(zb, rv[k], bb_ * pv[k]);
                     }
-                    store_vec_cs(xp, Vh, e, xv);
-                    store_vec_cs(pp, Vh, e, pv);
+                    store_vec_pol(x_base, Vh, e, xv, pol_base);
+                    if (p_s.res) p_s.s.store(slot, pv);
+                    store_vec(p_base, Vh, e, pv);
+                }
+                // the other live shifts of this iteration: deferred, worked off at the sync points that follow
+                pn = sc[rhs].nlive; pj = 0; ppass = 0;
+                pnpass = pn > 0 ? (ns + LS - 1) / LS : 0;
+            }
+            __syncthreads();                               // every thread has read sc[].done / coefficients
+            if (tid == 0) {
+                int n = 0;
+                for (int s = 0; s < R; ++s) {
+                    if (sc[s].done == 1) sc[s].done = 2;   // its last x/p update is queued
+                    n += sc[s].done == 0;
+                }
+                n_running = n;
+            }
+        }
+        STAG_TICK(2 * phase);
+
+        // ---- sync point: arrive, then work off deferred items until everybody needed has arrived -----------
+        // grid-wide after B and C (the two reductions): monotone counter `bar`.  After A and D a CTA needs w /
+        // p_base only from the CTAs that own its neighbouring sites (nb_list; all CTAs if cg_nbflags = 0): their
+        // epoch flags.  That is safe because two grid-wide barriers separate every write of w or p_base from the
+        // previous iteration's reads of it.  Warp 0 polls (relaxed loads, one flag per lane), issues the acquire
+        // fence once everybody needed has arrived (it also drops the SM's L1) and publishes the sync count in
+        // shared memory; the other warps work off their own pending items — thread-private sites, so no CTA
+        // barrier between items — until they see it or run out of items.  The closing CTA barrier hands warp 0's
+        // acquire on to them.
+        // Pending items MUST be finished (force) before phase D rewrites their coefficients, before phase C when
+        // it overwrites the r they read (no swap), at the end of the solve — and at once if filling is off.
+        {
+            const bool global = phase == 1 || phase == 2;
+            __syncthreads();                               // this phase's writes are issued; n_running is visible
+            const bool force = !a.fill || phase == 2 || (phase == 1 && !swap_rq) || (phase == 3 && n_running == 0);
+            const unsigned int sync_id = gepoch + nepoch + 1u;
+            unsigned int target;
+            if (global) {
+                target = ++gepoch * (unsigned)G;
+                if (tid == 0) { __threadfence(); atomicAdd(bar, 1u); }
+            } else {
+                target = ++nepoch;
+                if (tid == 0) {
+                    __threadfence();
+                    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" :: "l"(a.flags + (size_t)blockIdx.x * 32), "r"(target) : "memory");
                 }
             }
-        }
-        __syncthreads();                               // every thread has read sc[].done / coefficients
-        if (tid == 0) {
-            int n = 0;
-            for (int s = 0; s < R; ++s) {
-                if (sc[s].done == 1) sc[s].done = 2;   // its last x/p update has just run
-                n += sc[s].done == 0;
+            const bool poll_warp = tid < 32;
+            bool released = false;
+            while (!released || (force && ppass < pnpass)) {
+                unsigned int v = target;
+                if (poll_warp && !released) {
+                    if (global) {
+                        if (tid == 0) asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+                    } else {
+                        for (int c = tid; c < nnb; c += 32) {      // wrapped unsigned min over this lane's flags
+                            unsigned int f;
+                            asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];"
+                                         : "=r"(f) : "l"(a.flags + (size_t)nb_list[c] * 32) : "memory");
+                            if ((int)(f - v) < 0) v = f;
+                        }
+                    }
+                }
+                if (ppass < pnpass) {                      // one item; the poll is in flight meanwhile
+                    const Scalars<T> &c = sc[rhs];
+                    const int ls = l0 + ppass * LS;
+                    if (ls < ns) {
+                        const int e = e0 + ls, slot = rhs * S + ls, i = c.live[pj];
+                        const uint64_t pol = shift_policy(i);
+                        const T aj = c.ca[pj], zj = c.cz[pj], bj = c.cb[pj];
+                        T rv[6], pv[6], xv[6];
+                        r_s.load(slot, rhs, Vh, e, rv);
+                        load_vec_pol(p_r + (size_t)i * a.p_stride, Vh, e, pv, pol);
+                        load_vec_pol(x_r + (size_t)i * a.x_stride, Vh, e, xv, pol);
+#pragma unroll
+                        for (int k = 0; k < 6; ++k) {
+                            xv[k] = fma(aj, pv[k], xv[k]);
+                            pv[k] = fma(zj, rv[k], bj * pv[k]);
+                        }
+                        store_vec_pol(x_r + (size_t)i * a.x_stride, Vh, e, xv, pol);
+                        store_vec_pol(p_r + (size_t)i * a.p_stride, Vh, e, pv, pol);
+                    }
+                    if (++pj >= pn) { pj = 0; ++ppass; }
+                }
+                if (poll_warp) {
+                    if (!released && __all_sync(0xffffffffu, (int)(v - target) >= 0)) {
+                        if (tid == 0) {
+                            asm volatile("fence.acquire.gpu;" ::: "memory");
+                            *reinterpret_cast<volatile unsigned int *>(&sync_seen) = sync_id;
+                        }
+                        released = true;
+                    }
+                } else {
+                    // the other warps: released once warp 0 has seen the arrivals, or when out of items (the
+                    // closing CTA barrier then waits in hardware instead of spinning)
+                    released = ppass >= pnpass || *reinterpret_cast<volatile unsigned int *>(&sync_seen) == sync_id;
+                }
             }
-            n_running = n;
+            __syncthreads();
         }
-        STAG_TICK(7);
-        grid_wait(bar, ++epoch * G);                   // ends with __syncthreads: n_running, done visible
-        STAG_TICK(8);
+        STAG_TICK(2 * phase + 1);
+        phase = (phase + 1) & 3;
     }
 
     STAG_T_REPORT(R, sc[0].iter)
@@ -583,7 +741,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             for (int i = 0; i < nshift; ++i) {
                 const T ri = (T)st->residues[i];
                 T xv[6];
-                load_vec_cs(x_r + (size_t)i * a.x_stride, Vh, e, xv);
+                load_vec_pol(x_r + (size_t)i * a.x_stride, Vh, e, xv, policy_evict_first());
 #pragma unroll
                 for (int k = 0; k < 6; ++k) acc[k] = fma(ri, xv[k], acc[k]);
             }
@@ -614,20 +772,48 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
 // ---- host side ---------------------------------------------------------------------------------------
 static constexpr size_t kMaxDynSmem = 200 * 1024;     // of 227 KB; the rest: static scalars + L1
 
-// sites per CTA for a grid of `grid` CTAs (multiple of 32: every CTA's slice starts on a 512-byte line)
+// sites per CTA for a grid of `grid` CTAs (multiple of 32: every CTA's slice starts on a 512-byte line);
+// the slice layout of the mixed-precision kernel, and the slot count of a resident slice here (the largest CTA)
 inline int sites_per_cta(int Vh, int grid) {
     const int s = (Vh + grid - 1) / grid;
     return (s + 31) & ~31;
+}
+inline int persist_grid(const stag_ctx *ctx) {
+    const int tiles = (ctx->g.Vh + 31) / 32;
+    return ctx->num_sms < tiles ? ctx->num_sms : tiles;
+}
+inline int persist_slots(const stag_ctx *ctx) {       // sites of the largest CTA
+    const int tiles = (ctx->g.Vh + 31) / 32, grid = persist_grid(ctx);
+    return 32 * ((tiles + grid - 1) / grid);
+}
+
+// The shifts whose x_i, p_i the kernel marks evict_last: lightest first (they stay live longest), as many as
+// fit in `cg_l2_keep_mb` MB for all the sources of the launch.
+inline unsigned persist_keep_mask(const stag_ctx *ctx, int prec, int nrhs, int nshift, const double *shifts) {
+    const size_t per_shift = (size_t)2 * nrhs * ctx->g.Vh * vec_bytes_per_site(prec);
+    long long budget = (long long)ctx->opt.cg_l2_keep_mb << 20;
+    unsigned mask = 0;
+    for (;;) {
+        int best = -1;
+        for (int i = 0; i < nshift; ++i)
+            if (!((mask >> i) & 1u) && (best < 0 || shifts[i] < shifts[best])) best = i;
+        if (best < 0 || (long long)per_shift > budget) break;
+        budget -= (long long)per_shift;
+        mask |= 1u << best;
+    }
+    return mask;
 }
 
 template <typename T, int RECON, int NT, int R, bool SPLIT = false>
 int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t st) {
     const Geom &g = ctx->g;
-    int grid = ctx->num_sms;
-    const int tiles = (g.Vh + 31) / 32;
-    if (grid > tiles) grid = tiles;
+    const int grid = persist_grid(ctx);
+    if (grid > kMaxPersistGrid) return STAG_ERR_UNSUPPORTED;
     PersistArgs a = args;
-    a.S = sites_per_cta(g.Vh, grid);
+    a.S = persist_slots(ctx);
+    a.fill = ctx->opt.cg_fill != 0;
+    a.nbflags = ctx->opt.cg_nbflags != 0;
+
     // residency: as many of r, q, p (in that order of bytes saved) as fit
     const size_t slice = (size_t)a.S * R * 6 * sizeof(T);
     // cg_resident_slices (test / tuning knob): cap on how many of r, q, p stay in shared memory (default 3)
@@ -640,6 +826,7 @@ int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t
     int per_sm = 0;
     STAG_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
     if (per_sm < 1) return STAG_ERR_UNSUPPORTED;
+    STAG_CUDA_OK(cudaMemsetAsync(a.flags, 0, (size_t)grid * 128, st));
     Geom gg = g;
     void *params[] = {(void *)&gg, (void *)&a};
     STAG_CUDA_OK(cudaLaunchCooperativeKernel((const void *)kern, dim3(grid), dim3(NT), params, smem, st));
