@@ -1,21 +1,29 @@
 #!/usr/bin/env python
 """bench.py — staggered Dslash + multi-shift CG on B200 (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c5|c3|c2] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c4|c5|c3|c2|t2b|t2c] [--impl reference]
 
 One STEP = one pass of the whole hot path over one synthetic
 pseudo-fermion source: one multi-shift CG solve of (m^2 - D_eo D_oe + sigma_i) x_i = b with all its
 Dslash applications, reductions, scalar recurrences and shift updates.  Row a1 (gauge pack) is
-setup, done once and reported as `pack_ms`.  `value` = Dslash GFLOP/s sustained through the solve
-(570 flop/site x 2 Dslash/iteration x iterations x Vh / time): the BASELINE metric's first figure
-measured over the whole path; the CG time-to-solution and the standalone Dslash sweep are beside it.
-Prints ONE JSON line (rank 0).
+setup, done once and reported as `pack_ms`.
+
+The BASELINE metric has three figures; all three are first-class keys of the ONE JSON line (rank 0):
+  value / dslash_gflops_through_solve   Dslash GFLOP/s (570 flop/site) sustained through the timed solves
+  dslash_gflops_standalone              the same kernel timed alone (100-launch ping-pong), fp64-18
+  cg_s_per_solve                        multi-shift CG time to solution
+`roofline` is the dominant kernel of the step; `roofline.also[]` carries one entry per other kernel this run
+timed — the Dslash storage variants, the fp32 / 12-real solves, the block (N1) kernel, the force (N4), and the
+64^4 section (config 5: the largest single-GPU configuration, multi-kernel CG path) — each with its own
+algorithmic bytes, live CUDA-event duration, and the DRAM traffic of the committed ncu capture of the kernel
+of that NAME (profiles/traffic.csv; `traffic_stale` if the run launched a kernel the capture does not know).
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import re
 import statistics
 import subprocess
 import sys
@@ -39,6 +47,7 @@ DSLASH_BYTES = {(0, 18): 1248, (0, 12): 864, (1, 18): 624, (1, 12): 432,   # SUR
 PREC_NAME = {0: "f64", 1: "f32", 2: "f64split"}
 VARIANTS = ((0, 18), (0, 12), (1, 18), (1, 12), (2, 18), (2, 12))
 NOMINAL_HBM_GBS = 8000.0                              # "8 TB/s roofline" of BASELINE.json:metric
+METRIC = "Dslash GFLOP/s (570 flop/site) sustained through the multi-shift CG solve; CG s/solve beside it"
 
 
 def measured_peak_gbs():
@@ -49,28 +58,98 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def committed_traffic(workload, variant, kernel="dslash"):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed `ncu
-    --set full` capture (profiles/traffic.csv; text written from the capture, never by this run)."""
+# ---------------------------------------------------------------------------------------------
+# committed ncu traffic, looked up by KERNEL NAME
+# ---------------------------------------------------------------------------------------------
+def norm_kernel(name: str) -> str:
+    """One spelling for a kernel name, whether it comes from ncu ("void stag::k<double, (int)18, (bool)0>(stag::Geom,
+    ...)") or from abi::__cxa_demangle via stag_kernel_log ("void stag::k<double, 18, false>(stag::Geom, ...)")."""
+    n = name.strip()
+    n = re.sub(r"^void\s+", "", n)
+    depth, cut = 0, len(n)
+    for i, ch in enumerate(n):                        # drop the parameter list: the first '(' outside <...>
+        if ch == "<":
+            depth += 1
+        elif ch == ">":
+            depth -= 1
+        elif ch == "(" and depth == 0:
+            cut = i
+            break
+    n = n[:cut]
+    n = re.sub(r"\((?:int|bool|unsigned int|unsigned|long)\)", "", n)
+    n = n.replace("stag::", "").replace(" ", "").replace("false", "0").replace("true", "1")
+    return n
+
+
+def load_traffic():
     import csv
-    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    rows = []
     try:
-        with open(path, newline="") as f:
+        with open(os.path.join(ROOT, "profiles", "traffic.csv"), newline="") as f:
             for row in csv.DictReader(f):
-                if row["workload"] == workload and row["variant"] == variant and kernel in row["kernel"]:
-                    return int(row["dram_bytes_per_launch"])
+                row["_k"] = norm_kernel(row["kernel"])
+                rows.append(row)
     except Exception:
         pass
-    return None
+    return rows
 
 
-def cg_bytes_per_site(prec, recon, iters, iters_shift):
-    """Algorithmic bytes of one solve per even site: per iteration 2 Dslash +
-    p re-read (a3) + r,q,r (a5) + r (a6), plus x_i,p_i read+write for every iteration shift i was live."""
+_TRAFFIC = None
+
+
+def committed_traffic(workload: str, kernel: str, variant: str = ""):
+    """(dram bytes per launch, stale flag).  The row must be for this workload and for a kernel of exactly the
+    name the run launched (`kernel` comes from stag_kernel_log); a capture of another build of the kernel — other
+    template arguments — is NOT returned: (None, True).  `variant` disambiguates rows of one kernel name whose
+    traffic depends on run-time arguments (e.g. the number of sources of the block kernel)."""
+    global _TRAFFIC
+    if _TRAFFIC is None:
+        _TRAFFIC = load_traffic()
+    k = norm_kernel(kernel)
+    for row in _TRAFFIC:
+        if row["workload"] == workload and row["_k"] == k and (not variant or row.get("variant", "") == variant):
+            return int(row["dram_bytes_per_launch"]), False
+    return None, True
+
+
+def launched(ctx, pattern: str) -> str:
+    """Name (as stag_kernel_log gives it) of the one kernel matching `pattern` launched since the last reset."""
+    names = [n for n in ctx.kernel_log() if re.search(pattern, n)]
+    return names[0] if names else "?"
+
+
+def roof_entry(workload, kernel, what, alg_bytes, secs_per_launch, peak, peak_src, variant="", **extra):
+    gbs = alg_bytes / secs_per_launch / 1e9
+    traffic, stale = committed_traffic(workload, kernel, variant)
+    e = {"bound": "hbm", "kernel": norm_kernel(kernel), "what": what, "workload": workload, "achieved": gbs, "peak": peak,
+         "unit": "GB/s", "frac": gbs / peak, "peak_source": peak_src, "frac_of_8tbs": gbs / NOMINAL_HBM_GBS,
+         "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": secs_per_launch * 1e6, "traffic": traffic}
+    if stale:
+        e["traffic_stale"] = True
+    elif traffic:
+        e["frac_dram"] = traffic / secs_per_launch / 1e9 / peak     # real HBM traffic of the capture / live time / peak
+    e.update(extra)
+    return e
+
+
+def cg_bytes_per_site(prec, recon, iters, iters_shift, resident=False):
+    """Algorithmic bytes of one solve per even site.  Multi-kernel path, per iteration: 2 Dslash
+    + p re-read (a3) + r,q,r (a5) + r (a6), plus x_i,p_i read+write for every iteration shift i was live:
+    2D + 5 vec + 4 vec N.  resident = the persistent kernel with r, q, p_base in shared memory: q is never written
+    to memory, p, r, q are never re-read from it, and the base shift only writes p: 2D - 2 vec + 4 vec N."""
     w = 4 if prec == 1 else 8
     vec = 6 * w
-    per_iter = 2 * DSLASH_BYTES[(prec, recon)] + vec + 3 * vec + vec
+    per_iter = 2 * DSLASH_BYTES[(prec, recon)] + (-2 * vec if resident else 5 * vec)
     return iters * per_iter + sum(iters_shift) * 4 * vec
+
+
+def fully_resident(vh, prec, num_sms=148):
+    """Mirror of launch_persistent's residency rule (csrc/stag_cg_persist.cuh): r, q and p_base all in shared memory."""
+    w = 4 if prec == 1 else 8
+    tiles = (vh + 31) // 32
+    grid = min(num_sms, tiles)
+    slots = 32 * ((tiles + grid - 1) // grid)
+    return 3 * slots * 6 * w <= 200 * 1024
 
 
 class ClockSampler:
@@ -178,9 +257,6 @@ def run_reference(args):
     return 0
 
 
-METRIC = "Dslash GFLOP/s (570 flop/site) sustained through the multi-shift CG solve; CG s/solve beside it"
-
-
 def workload_config(cfg, name, prec, recon):
     L = cfg["L"]
     return {"workload": "%s: %dx%dx%dx%d lattice, %s links, %d-shift multi-shift CG, m=%g, stop=%g, %d source(s)"
@@ -252,13 +328,92 @@ def time_dslash(torch, ctx, packed, prec, recon, a, b, launches=100, repeats=5, 
     return time_launches(torch, pair, launches, repeats)
 
 
-def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
+def timed_call(torch, fn, repeats=2):
+    """CUDA events around fn(); the LAST of `repeats` calls is the one reported (the others warm up)."""
+    out = None
+    for _ in range(repeats):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        out = fn()
+        e1.record()
+        torch.cuda.synchronize()
+    return e0.elapsed_time(e1) * 1e-3, out
+
+
+def dslash_variants(torch, stag, ctx, wl, U, srcs, vh, peak, peak_src, launches, have=None):
+    """The Dslash bandwidth sweep over the storage variants; returns (table, roofline entries)."""
+    table, entries = {}, []
+    canon = None
+    for p_, r_ in VARIANTS:
+        if have is not None and (p_, r_) in have:
+            pk = have[(p_, r_)]
+        else:
+            if canon is None:
+                canon = ctx.alloc(ctx.gauge_canonical_bytes())
+                ctx.gauge_load(U, canon)
+                torch.cuda.synchronize()
+            pk = ctx.alloc(ctx.gauge_packed_bytes(p_, r_))
+            ctx.gauge_pack(canon, pk, p_, r_)
+        vp = stag.F32 if p_ == stag.F32 else stag.F64
+        a, b = ctx.upload_vector(srcs[0], vp), ctx.alloc(ctx.vector_bytes(vp))
+        ctx.kernel_log_reset()
+        s_per = time_dslash(torch, ctx, pk, p_, r_, a, b, launches=launches)
+        kern = launched(ctx, r"dslash_kernel")
+        name = "%s-%d" % (PREC_NAME[p_], r_)
+        gbs = DSLASH_BYTES[(p_, r_)] * vh / s_per / 1e9
+        table[name] = {"us": s_per * 1e6, "gflops": FLOP_PER_SITE * vh / s_per / 1e9, "gbs_algorithmic": gbs,
+                       "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak,
+                       "bytes_per_site": DSLASH_BYTES[(p_, r_)]}
+        entries.append(roof_entry(wl, kern, "stag_dslash_oe/eo %s, %d launches ping-pong replayed as a CUDA graph" % (name, launches),
+                                  DSLASH_BYTES[(p_, r_)] * vh, s_per, peak, peak_src, variant=name,
+                                  gflops=FLOP_PER_SITE * vh / s_per / 1e9))
+        del pk, a, b
+    del canon
+    return table, entries
+
+
+def measure_solve(torch, stag, ctx, wl, cfg, packed, prec, recon, src, vh, peak, peak_src, stop=None, warm=1, opts=()):
+    """One timed stag_mshift_cg solve (after `warm` untimed ones) of a storage variant; returns (dict, roofline entry)."""
+    shifts, n = cfg["shifts"], len(cfg["shifts"])
+    vp = stag.F32 if prec == stag.F32 else stag.F64
+    vb = ctx.vector_bytes(vp)
+    b = ctx.upload_vector(src, vp)
+    x, ws = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(prec, n))
+    stop = cfg["stops"][0] if stop is None else stop
+    ctx.kernel_log_reset()
+    secs, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg(packed, prec, recon, b, cfg["mass"], shifts, stop, 100000, x, ws),
+                                  repeats=warm + 1)
+    persistent = info["kernel_launches"] == 1
+    name = "%s-%d" % (PREC_NAME[prec], recon)
+    resident = persistent and fully_resident(vh, prec)
+    own = cg_bytes_per_site(prec, recon, info["iters"], info["iters_shift"], resident) * vh
+    equiv = cg_bytes_per_site(prec, recon, info["iters"], info["iters_shift"], False) * vh
+    d = {"rc": rc, "s_per_solve": secs, "iters": info["iters"], "us_per_iter": secs / max(info["iters"], 1) * 1e6,
+         "converged": info["converged"], "stagnated": info["stagnated"], "path": "persistent" if persistent else "multi-kernel",
+         "gflops_through_solve": 2 * FLOP_PER_SITE * vh * info["iters"] / secs / 1e9,
+         "gbs_algorithmic": own / secs / 1e9, "pct_of_measured": 100 * own / secs / 1e9 / peak,
+         "equivalent_gbs": equiv / secs / 1e9, "sum_iters_shift": sum(info["iters_shift"])}
+    if persistent:
+        kern = launched(ctx, r"cg_persistent_kernel")
+        e = roof_entry(wl, kern, "stag_mshift_cg %s: one launch = one %d-shift solve (%d iterations)" % (name, n, info["iters"]),
+                       own, secs, peak, peak_src, variant=name, iters=info["iters"], us_per_iter=d["us_per_iter"],
+                       equivalent_gbs=equiv / secs / 1e9,
+                       bytes_model="2D - 2 vec + 4 vec N_live per site and iteration (r, q, p_base in shared memory)"
+                       if resident else "2D + 5 vec + 4 vec N_live per site and iteration")
+    else:
+        e = None
+    return d, e
+
+
+def measure_block(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak, peak_src):
     """N1: stag_dslash_block for R = 1, 2, 4 sources (100-launch ping-pong, as time_dslash) and ONE
     stag_mshift_cg_block solve of min(4, nsrc) sources.  Algorithmic bytes per site of a block Dslash =
     8 links (once) + R x (one read of the source + one write)."""
     w = 4 if prec == stag.F32 else 8
     vb = ctx.vector_bytes(prec)
     out = {"dslash": {}, "cg": None}
+    entries = []
+    name = "%s-%d" % (PREC_NAME[prec], recon)
     for R in (1, 2, 4):
         if R > len(srcs):
             continue
@@ -269,12 +424,17 @@ def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
                 ctx.dslash_block(packed, prec, recon, 1, R, a, b)
                 ctx.dslash_block(packed, prec, recon, 0, R, b, a)
         pair(10)
+        ctx.kernel_log_reset()
         s_per = time_launches(torch, pair, 100)
         bps = 8 * recon * w + 2 * 6 * w * R
         gbs = bps * vh / s_per / 1e9
         out["dslash"]["R%d" % R] = {"us": s_per * 1e6, "us_per_source": s_per * 1e6 / R,
                                     "gflops": FLOP_PER_SITE * vh * R / s_per / 1e9, "bytes_per_site": bps,
                                     "gbs_algorithmic": gbs, "pct_of_measured": 100 * gbs / peak}
+        if R == 4:
+            entries.append(roof_entry(wl, launched(ctx, r"dslash_(pipe|block)_kernel"),
+                                      "stag_dslash_block %s, 4 sources through one link read" % name, bps * vh, s_per,
+                                      peak, peak_src, variant=name + "-R4", gflops=FLOP_PER_SITE * vh * 4 / s_per / 1e9))
         del a, b
     R = min(4, len(srcs))
     n = len(cfg["shifts"])
@@ -282,20 +442,23 @@ def measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak):
     bdev = ctx.upload_vectors(srcs[:R], prec)
     x = ctx.alloc(R * n * vb)
     ws = ctx.alloc(ctx.cg_block_workspace_bytes(prec, n, R))
-    ts = []
-    for _ in range(2):                                    # first = warm-up
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        rc, infos = ctx.mshift_cg_block(packed, prec, recon, R, bdev, cfg["mass"], cfg["shifts"], stop, 100000, x, ws)
-        e1.record()
-        torch.cuda.synchronize()
-        ts.append(e0.elapsed_time(e1) * 1e-3)
+    ctx.kernel_log_reset()
+    secs, (rc, infos) = timed_call(torch, lambda: ctx.mshift_cg_block(packed, prec, recon, R, bdev, cfg["mass"], cfg["shifts"],
+                                                                      stop, 100000, x, ws))
     its = [i["iters"] for i in infos]
-    out["cg"] = {"nrhs": R, "rc": rc, "s_per_block_solve": ts[-1], "s_per_source": ts[-1] / R, "iters": its,
-                 "us_per_iter": ts[-1] / max(its) * 1e6, "stop": stop,
-                 "gflops": 2 * FLOP_PER_SITE * vh * sum(its) / ts[-1] / 1e9,
+    # per source and iteration: links / R twice + the vector traffic of the multi-kernel formula (nothing of q, p
+    # is resident at R = 4; r is) — reported with the single-source multi-kernel formula so that it compares
+    vec = 6 * w
+    alg = vh * sum(i["iters"] * (2 * (8 * recon * w / R + 2 * vec) + 5 * vec) + sum(i["iters_shift"]) * 4 * vec for i in infos)
+    out["cg"] = {"nrhs": R, "rc": rc, "s_per_block_solve": secs, "s_per_source": secs / R, "iters": its,
+                 "us_per_iter": secs / max(its) * 1e6, "stop": stop,
+                 "gflops": 2 * FLOP_PER_SITE * vh * sum(its) / secs / 1e9,
+                 "gbs_algorithmic": alg / secs / 1e9, "pct_of_measured": 100 * alg / secs / 1e9 / peak,
                  "call": "stag_mshift_cg_block (one persistent launch, links read once per Dslash for all sources)"}
-    return out
+    entries.append(roof_entry(wl, launched(ctx, r"cg_persistent_kernel"),
+                              "stag_mshift_cg_block %s: one launch = %d sources x %d shifts" % (name, R, n), alg, secs,
+                              peak, peak_src, variant=name + "-R%d" % R, us_per_iter=out["cg"]["us_per_iter"]))
+    return out, entries
 
 
 def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
@@ -310,14 +473,8 @@ def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
     ws = ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(n))
     out = {}
     for name, hi, prec_hi, lo in (("split_buffer", split, stag.F64_SPLIT, split), ("f64_polish_f32_inner", p64, stag.F64, split)):
-        for _ in range(2):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            rc, info = ctx.mshift_cg_mixed(hi, prec_hi, 18, lo, 18, b, cfg["mass"], cfg["shifts"], cfg["stops"][0],
-                                           100000, x, ws)
-            e1.record()
-            torch.cuda.synchronize()
-        secs = e0.elapsed_time(e1) * 1e-3
+        secs, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(hi, prec_hi, 18, lo, 18, b, cfg["mass"], cfg["shifts"],
+                                                                         cfg["stops"][0], 100000, x, ws))
         out[name] = {"rc": rc, "s_per_solve": secs, "vs_fp64_multishift": fp64_s_per_solve / secs,
                      "inner_fp32_iters": info["inner"]["iters"], "polish_iters": info["polish"]["iters"],
                      "polish_passes": info["polish"]["passes"],
@@ -328,21 +485,10 @@ def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
     # TRUE fp64 residual, nothing is left to polish; the fp64 solver on the same single system beside it
     sh1 = cfg["shifts"][:1]
     cgws = ctx.alloc(ctx.cg_workspace_bytes(stag.F64, 1))
-    for _ in range(2):
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        rc64, i64 = ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], sh1, cfg["stops"][0], 100000, x, cgws)
-        e1.record()
-        torch.cuda.synchronize()
-    t64 = e0.elapsed_time(e1) * 1e-3
-    for _ in range(2):
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        # fp32 iterations on the b planes, fp64 residual replacement on b + c of the SAME split-double buffer (N3)
-        rc, info = ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], sh1, cfg["stops"][0], 100000, x, ws)
-        e1.record()
-        torch.cuda.synchronize()
-    tm = e0.elapsed_time(e1) * 1e-3
+    t64, (rc64, i64) = timed_call(torch, lambda: ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], sh1, cfg["stops"][0], 100000, x, cgws))
+    # fp32 iterations on the b planes, fp64 residual replacement on b + c of the SAME split-double buffer (N3)
+    tm, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], sh1,
+                                                                   cfg["stops"][0], 100000, x, ws))
     out["single_shift_residual_replacement"] = {
         "rc": rc, "s_per_solve": tm, "fp64_s_per_solve": t64, "vs_fp64": t64 / tm, "iters": info["inner"]["iters"],
         "fp64_iters": i64["iters"], "reliable_updates": info["reliable_updates"],
@@ -350,7 +496,7 @@ def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
     return out
 
 
-def measure_force(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh):
+def measure_force(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak, peak_src):
     """N4: stag_fermion_force on nshift even vectors (the x_i of a solve; timing does not depend on their
     values, so the sources stand in), 20 calls between CUDA events after 3 warm-up calls.  Algorithmic bytes:
     D_oe x_i through the multi-source kernel (links once per group of 4, each vector read + written once) +
@@ -363,6 +509,7 @@ def measure_force(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh):
     res = [1.0 / (i + 1) for i in range(n)]
     for _ in range(3):
         ctx.fermion_force(packed, prec, recon, res, x, F, ws)
+    ctx.kernel_log_reset()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
     e0.record()
@@ -375,30 +522,96 @@ def measure_force(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh):
     bytes_dslash = vh * (groups * 8 * recon * w + n * 2 * 6 * w)
     bytes_force = 2 * vh * (4 * recon * w + 4 * 144 + n * 6 * w)
     gbs = (bytes_dslash + bytes_force) / secs / 1e9
-    return {"us_per_call": secs * 1e6, "nshift": n, "launches_per_call": 1 + groups,
-            "algorithmic_bytes_per_call": bytes_dslash + bytes_force, "gbs_algorithmic": gbs}
+    # the D_oe launches of the call, timed alone, so that the force kernel proper gets its own figure
+    vb = ctx.vector_bytes(prec)
+
+    def dsl(k):
+        for _ in range(k):
+            for g in range(groups):
+                ctx.dslash_block(packed, prec, recon, 1, min(4, n - 4 * g), x[4 * g * vb:], ws[4 * g * vb:])
+    dsl(2)
+    s_dsl = time_launches(torch, dsl, 10)
+    s_force = max(secs - s_dsl, 1e-9)
+    name = "%s-%d" % (PREC_NAME[prec], recon)
+    d = {"us_per_call": secs * 1e6, "nshift": n, "launches_per_call": 1 + groups, "us_dslash_launches": s_dsl * 1e6,
+         "us_force_kernel": s_force * 1e6, "algorithmic_bytes_per_call": bytes_dslash + bytes_force,
+         "gbs_algorithmic": gbs, "pct_of_measured": 100 * gbs / peak}
+    e = roof_entry(wl, launched(ctx, r"force_kernel"),
+                   "stag_fermion_force %s, %d shifts: the force kernel proper (call minus its %d D_oe launches, timed alone)"
+                   % (name, n, groups), bytes_force, s_force, peak, peak_src, variant=name, us_per_call=secs * 1e6,
+                   call_gbs_algorithmic=gbs, call_frac=gbs / peak)
+    return d, e
 
 
-def dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, pack_ms, gen_s):
-    """--dslash-only: the SURVEY.md §8(d) Dslash bandwidth sweep alone (no CG), one JSON line."""
-    peak, peak_src = measured_peak_gbs()
-    del packed
+def c5_section(torch, stag, args, peak, peak_src):
+    """Config 5 (64^4: the largest single-GPU configuration of BASELINE.json:configs; the multi-kernel CG path):
+    the Dslash sweep, ONE timed 8-shift solve after a 32-iteration warm-up call, and the four kernels of an
+    iteration timed one by one with CUDA events (option cg_profile, a separate 48-iteration call)."""
+    import stag_inputs as si
+    wl = "c5"
+    cfg = si.get_config(WORKLOADS[wl])
+    L, vh = cfg["L"], int(np.prod(cfg["L"])) // 2
+    U, srcs, gen_s = make_inputs(cfg)
+    ctx = stag.Stag(L)
+    for kv in args.opt:
+        k, v = kv.split("=")
+        ctx.set_option(k, int(v))
     canon = ctx.alloc(ctx.gauge_canonical_bytes())
     ctx.gauge_load(U, canon)
     torch.cuda.synchronize()
+    p64 = ctx.alloc(ctx.gauge_packed_bytes(stag.F64, 18))
+    secs_pack, _ = timed_call(torch, lambda: ctx.gauge_pack(canon, p64, stag.F64, 18), repeats=1)
+    del canon
+    out = {"workload": WORKLOADS[wl], "input_gen_s": gen_s, "pack_ms": secs_pack * 1e3, "vh": vh}
+    entries = []
+    # ---- CG: fp64-18, 8 shifts, stop 1e-9
+    shifts, n = cfg["shifts"], len(cfg["shifts"])
+    vb = ctx.vector_bytes(stag.F64)
+    b = ctx.upload_vector(srcs[0], stag.F64)
+    x, ws = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(stag.F64, n))
+    ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], shifts, cfg["stops"][0], 32, x, ws)          # warm-up: 32 iterations
+    ctx.kernel_log_reset()
+    secs, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], shifts, cfg["stops"][0],
+                                                               100000, x, ws), repeats=1)
+    alg = cg_bytes_per_site(0, 18, info["iters"], info["iters_shift"]) * vh
+    out["cg"] = {"rc": rc, "s_per_solve": secs, "iters": info["iters"], "us_per_iter": secs / max(info["iters"], 1) * 1e6,
+                 "gflops_through_solve": 2 * FLOP_PER_SITE * vh * info["iters"] / secs / 1e9,
+                 "gbs_algorithmic": alg / secs / 1e9, "pct_of_measured": 100 * alg / secs / 1e9 / peak,
+                 "kernel_launches": info["kernel_launches"], "iters_shift": info["iters_shift"],
+                 "path": "multi-kernel (4 launches per iteration, CUDA-graph replay)"}
+    names = ctx.kernel_log()
+    pick = lambda pat: next((k for k in names if re.search(pat, k)), "?")
+    k_a2, k_a3 = pick(r"dslash_kernel<.*, ?1, ?\d+, ?(false|0)>"), pick(r"dslash_kernel<.*, ?2, ?\d+, ?(false|0)>")
+    k_a5, k_a6 = pick(r"cg_update_r_kernel"), pick(r"cg_update_shifts_kernel")
+    # the four kernels one by one (first 40 iterations: every shift still live)
+    ctx.set_option("cg_profile", 1)
+    ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], shifts, cfg["stops"][0], 48, x, ws)
+    ctx.set_option("cg_profile", 0)
+    us, nit = ctx.cg_profile()
+    out["cg"]["profile_us"] = {"a2_dslash_oe": us[0], "a3_dslash_eo_fused": us[1], "a5_update_r": us[2], "a6_update_shifts": us[3],
+                               "iterations_averaged": nit, "live_shifts": n}
+    if nit > 0:
+        vec = 48
+        for kern, what, bytes_site, t in ((k_a2, "a2: w = D_oe p", 1248, us[0]), (k_a3, "a3: q = c0 p - D_eo w, <p,q>", 1248 + vec, us[1]),
+                                          (k_a5, "a5: r -= alpha q, <r,r>", 3 * vec, us[2]),
+                                          (k_a6, "a6: all-shift update, %d live shifts" % n, vec + 4 * vec * n, us[3])):
+            entries.append(roof_entry(wl, kern, "stag_mshift_cg f64-18 multi-kernel path, " + what + " (CUDA events around each launch)",
+                                      bytes_site * vh, t * 1e-6, peak, peak_src, variant="f64-18"))
+    del x, ws, b
+    # ---- Dslash sweep
+    table, ents = dslash_variants(torch, stag, ctx, wl, U, srcs, vh, peak, peak_src, args.dslash_launches,
+                                  have={(stag.F64, 18): p64})
+    out["dslash"] = table
+    return out, ents + entries
+
+
+def dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, vh, pack_ms, gen_s):
+    """--dslash-only: the SURVEY.md §8(d) Dslash bandwidth sweep alone (no CG), one JSON line."""
+    peak, peak_src = measured_peak_gbs()
+    table, entries = dslash_variants(torch, stag, ctx, args.workload, U, srcs, vh, peak, peak_src, args.dslash_launches)
     out = {"metric": "Dslash GFLOP/s & HBM GB/s", "workload": WORKLOADS[args.workload], "peak_gbs": peak,
-           "peak_source": peak_src, "pack_ms": pack_ms, "input_gen_s": gen_s, "dslash": {}}
-    for p_, r_ in VARIANTS:
-        pk = ctx.alloc(ctx.gauge_packed_bytes(p_, r_))
-        ctx.gauge_pack(canon, pk, p_, r_)
-        a = ctx.upload_vector(srcs[0], p_)
-        b = ctx.alloc(ctx.vector_bytes(p_))
-        s_per = time_dslash(torch, ctx, pk, p_, r_, a, b, launches=args.dslash_launches)
-        gbs = DSLASH_BYTES[(p_, r_)] * vh / s_per / 1e9
-        out["dslash"]["%s-%d" % (PREC_NAME[p_], r_)] = {
-            "us": s_per * 1e6, "gflops": FLOP_PER_SITE * vh / s_per / 1e9, "gbs_algorithmic": gbs,
-            "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak}
-        del pk, a, b
+           "peak_source": peak_src, "pack_ms": pack_ms, "input_gen_s": gen_s, "dslash": table,
+           "roofline": {"also": entries}}
     if args.workload in PAPER_TABLE2:
         pg, pb, cite = PAPER_TABLE2[args.workload]
         ours = out["dslash"]["f32-12"]
@@ -424,11 +637,14 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     prec = {"f64": stag.F64, "f32": stag.F32, "f64split": stag.F64_SPLIT}[args.prec]
     recon = args.recon
-    cfg = si.get_config(WORKLOADS[args.workload])
+    wl = args.workload
+    cfg = si.get_config(WORKLOADS[wl])
     L = cfg["L"]
     vh = int(np.prod(L)) // 2
     shifts, nshift = cfg["shifts"], len(cfg["shifts"])
     stop, maxiter = cfg["stops"][0], 100000
+    peak, peak_src = measured_peak_gbs()
+    vprec = stag.F32 if prec == stag.F32 else stag.F64
 
     # ---- setup (a1): seeded synthetic inputs -> HBM, packed once --------------------------------
     U, srcs, gen_s = make_inputs(cfg)
@@ -447,16 +663,17 @@ def run_ours(args):
     torch.cuda.synchronize()
     pack_ms = e0.elapsed_time(e1)
     del canon
-    vb = ctx.vector_bytes(prec)
+    vb = ctx.vector_bytes(vprec)
     if args.dslash_only:
-        return dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, packed, prec, recon, vh, pack_ms, gen_s)
-    bdev = [ctx.upload_vector(s, prec) for s in srcs]
+        del packed
+        return dslash_sweep(args, torch, stag, ctx, cfg, U, srcs, vh, pack_ms, gen_s)
+    bdev = [ctx.upload_vector(s, vprec) for s in srcs]
     x = ctx.alloc(nshift * vb)
     ws = ctx.alloc(ctx.cg_workspace_bytes(prec, nshift))
 
     def solve(k):
         rc, info = ctx.mshift_cg(packed, prec, recon, bdev[k], cfg["mass"], shifts, stop, maxiter, x, ws)
-        if rc != 0:
+        if rc != 0 and not (prec == stag.F32 and rc == stag.ERR_NOTCONV):
             raise RuntimeError("stag_mshift_cg rc=%d %r" % (rc, info))
         return info
 
@@ -472,6 +689,7 @@ def run_ours(args):
     barrier()
     if rank == 0:
         clocks.start()
+    ctx.kernel_log_reset()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     infos = []
     e0.record()
@@ -480,10 +698,14 @@ def run_ours(args):
     e1.record()
     barrier()
     clk = clocks.stop() if rank == 0 else None
-    secs, (tot_iters, tot_bytes_site, launches) = reduce_over_ranks(
+    step_kernels = ctx.kernel_log()
+    persistent = all(i["kernel_launches"] == 1 for i in infos)
+    resident = persistent and fully_resident(vh, prec)
+    secs, (tot_iters, own_bytes_site, equiv_bytes_site, launches) = reduce_over_ranks(
         torch, dist, world, e0.elapsed_time(e1) * 1e-3,
         [sum(i["iters"] for i in infos),
-         sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"]) for i in infos),
+         sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"], resident) for i in infos),
+         sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"], False) for i in infos),
          sum(i["kernel_launches"] for i in infos)], "cuda")
     value = 2 * FLOP_PER_SITE * vh * tot_iters / secs / 1e9
     nsolves = args.steps * world
@@ -509,89 +731,101 @@ def run_ours(args):
     e2e_value = 2 * FLOP_PER_SITE * vh * ie_sum / te_s / 1e9
     del scratch, hx
 
-    # ---- roofline of the dominant kernel (the Dslash) and the sweep over storage variants ---------
-    peak, peak_src = measured_peak_gbs()
-    dslash = {}
-    roof = roof_dslash = None
+    out = None
     if rank == 0:
-        va, vb_ = ctx.alloc(ctx.vector_bytes(stag.F64)), ctx.alloc(ctx.vector_bytes(stag.F64))
-        for p_, r_ in VARIANTS:
-            pk = packed if (p_, r_) == (prec, recon) else ctx.upload_gauge(U, p_, r_)
-            a = ctx.upload_vector(srcs[0], p_)
-            s_per = time_dslash(torch, ctx, pk, p_, r_, a, vb_ if p_ != stag.F32 else va)
-            gbs = DSLASH_BYTES[(p_, r_)] * vh / s_per / 1e9
-            dslash["%s-%d" % (PREC_NAME[p_], r_)] = {
-                "us": s_per * 1e6, "gflops": FLOP_PER_SITE * vh / s_per / 1e9, "gbs_algorithmic": gbs,
-                "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak,
-                "bytes_per_site": DSLASH_BYTES[(p_, r_)]}
-            if (p_, r_) == (prec, recon):
-                roof = {"bound": "hbm", "kernel": "dslash_kernel<%s,%d> (stag_dslash_oe/eo, %d launches ping-pong)"
-                        % ("float" if p_ == stag.F32 else "double", r_, 100),
-                        "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak,
-                        "peak_source": peak_src, "frac_of_8tbs": gbs / NOMINAL_HBM_GBS,
-                        "algorithmic_bytes_per_launch": DSLASH_BYTES[(p_, r_)] * vh,
-                        "avg_launch_us": s_per * 1e6, "traffic": None}
-            if pk is not packed:
+        also = []
+        name = "%s-%d" % (PREC_NAME[prec], recon)
+        # ---- roofline of the step's dominant kernel ------------------------------------------------
+        if persistent:
+            # the whole solve is ONE kernel (stag_cg_persist.cuh): that kernel is the step.  `achieved` uses the
+            # bytes THIS kernel has to move (r, q, p_base stay in shared memory); the multi-kernel formula of
+            # SURVEY.md §8(d) is beside it as `equivalent_gbs`, and the real DRAM bytes of the ncu capture as `traffic`
+            roof = roof_entry(wl, next((k for k in step_kernels if "cg_persistent_kernel" in k), "?"),
+                              "stag_mshift_cg %s: one launch = one %d-shift solve" % (name, nshift),
+                              own_bytes_site * vh / nsolves, secs / args.steps, peak, peak_src, variant=name,
+                              equivalent_gbs=equiv_bytes_site * vh / secs / 1e9 / world,
+                              bytes_model=("2D - 2 vec + 4 vec N_live" if resident else "2D + 5 vec + 4 vec N_live")
+                              + " per even site and iteration, summed over the iterations of the solve")
+        else:
+            roof = None                                   # set from the Dslash sweep below (multi-kernel path)
+        # ---- Dslash sweep over the storage variants ---------------------------------------------------
+        dslash, ents = dslash_variants(torch, stag, ctx, wl, U, srcs, vh, peak, peak_src, args.dslash_launches,
+                                       have={(prec, recon): packed})
+        also += ents
+        if roof is None:
+            roof = next(e for e in ents if e.get("workload") == wl and name in e["what"])
+        # ---- the solve in the other storage variants (fp32 / 12-real need driver-visible figures) ----
+        solves = {}
+        if not args.no_block and prec == stag.F64 and recon == 18:
+            for p_, r_ in ((stag.F64, 12), (stag.F32, 18), (stag.F32, 12)):
+                pk = ctx.upload_gauge(U, p_, r_)
+                d, e = measure_solve(torch, stag, ctx, wl, cfg, pk, p_, r_, srcs[0], vh, peak, peak_src)
+                solves["%s-%d" % (PREC_NAME[p_], r_)] = d
+                if e:
+                    also.append(e)
                 del pk
-        roof["traffic"] = committed_traffic(args.workload, "%s-%d" % (args.prec, recon))
-        roof_dslash = roof
-        if launches == nsolves:
-            # the whole solve ran as ONE kernel per step (stag_cg_persist.cu): that kernel is the dominant
-            # one.  Algorithmic bytes per launch = SURVEY.md §8(d): (2736 + 192 N_live) per even site and
-            # iteration (fp64-18), summed over the iterations of the solve; duration = CUDA events around
-            # the K launches of the timed region / K.
-            cg_bytes_launch = tot_bytes_site * vh / nsolves
-            cg_gbs_ = tot_bytes_site * vh / secs / 1e9 / world        # per GPU: ranks run concurrently
-            roof = {"bound": "hbm", "kernel": "cg_persistent_kernel<%s,%d> (one launch = one multi-shift solve)"
-                    % ("float" if prec == stag.F32 else "double", recon),
-                    "achieved": cg_gbs_, "peak": peak, "unit": "GB/s", "frac": cg_gbs_ / peak,
-                    "peak_source": peak_src, "frac_of_8tbs": cg_gbs_ / NOMINAL_HBM_GBS,
-                    "algorithmic_bytes_per_launch": cg_bytes_launch, "avg_launch_us": secs / args.steps * 1e6,
-                    "traffic": committed_traffic(args.workload, "%s-%d" % (args.prec, recon), "cg_persistent")}
-
-    # ---- N1: the 4 pseudo-fermion sources of the workload through ONE link read ----
-    block = None
-    if rank == 0 and not args.no_block and len(srcs) >= 2 and prec != stag.F64_SPLIT:
-        block = measure_block(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh, peak)
-
-    # ---- N2/N3: fp32 multi-shift + fp64 polish on one split-double buffer -----------------------------
-    mixed = None
-    if rank == 0 and not args.no_block and prec == stag.F64:
-        mixed = measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, secs / args.steps)
-
-    force = None
-    if rank == 0 and not args.no_block and prec != stag.F64_SPLIT:
-        force = measure_force(torch, stag, ctx, cfg, srcs, packed, prec, recon, vh)
-        force["pct_of_measured"] = 100 * force["gbs_algorithmic"] / peak
-
-    # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
-    cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        g, s_it, m = oracle_sample(cfg, U, srcs[0], 12.0)
-        cpu = {"value": g, "unit": "GFLOP/s", "cores": 1, "kind": "oracle",
-               "sample": "%d oracle multi-shift CG iterations (maxiter=%d) of the same %d-shift solve, %.3f s/iteration"
-                         % (m, m, nshift, s_it)}
-
-    if rank == 0:
+        # ---- N1: the 4 pseudo-fermion sources of the workload through ONE link read ----------------------
+        block = mixed = force = None
+        if not args.no_block and len(srcs) >= 2 and prec != stag.F64_SPLIT:
+            block, ents = measure_block(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak, peak_src)
+            also += ents
+        # ---- N2/N3: fp32 multi-shift + fp64 polish on one split-double buffer -----------------------------
+        if not args.no_block and prec == stag.F64:
+            mixed = measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, secs / args.steps)
+        # ---- N4 ---------------------------------------------------------------------------------------------
+        if not args.no_block and prec != stag.F64_SPLIT:
+            force, e = measure_force(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak, peak_src)
+            also.append(e)
+        l2_bytes = torch.cuda.get_device_properties(local).L2_cache_size
+        wset = ctx.gauge_packed_bytes(prec, recon) + (2 * nshift + 4) * vb
         iters = [i["iters"] for i in infos]
-        cg_gbs = tot_bytes_site * vh / secs / 1e9
+        cg_gbs = own_bytes_site * vh / secs / 1e9
         out = {"metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": secs * 1e3 / args.steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.prec == "f32" else "f64", "data": "synthetic",
-               "config": dict(workload_config(cfg, args.workload, prec, recon),
-                              l2="working set (2 link sets + %d vectors = %.0f MB) larger than the 126 MB L2; no flush"
-                                 % (2 * nshift + 4, (ctx.gauge_packed_bytes(prec, recon) + (2 * nshift + 4) * vb) / 1e6)),
+               "config": dict(workload_config(cfg, wl, prec, recon),
+                              l2="working set (2 link sets + %d vectors) = %.0f MB %s the %.0f MB L2%s"
+                                 % (2 * nshift + 4, wset / 1e6, "exceeds" if wset > l2_bytes else "FITS in", l2_bytes / 1e6,
+                                    "; no flush between steps" if wset > l2_bytes else
+                                    ": an L2-resident run, not held to the HBM roofline")),
+               "dslash_gflops_through_solve": value,
+               "dslash_gflops_standalone": dslash[name]["gflops"],
+               "cg_s_per_solve": secs / args.steps,
                "cg": {"s_per_solve": secs / args.steps, "iters": iters, "us_per_iter": secs / (tot_iters / world) * 1e6,
+                      "path": "persistent" if persistent else "multi-kernel",
                       "gbs_algorithmic": cg_gbs, "pct_of_8tbs": 100 * cg_gbs / NOMINAL_HBM_GBS,
-                      "pct_of_measured": 100 * cg_gbs / peak, "solves": nsolves,
-                      "iters_shift_first_solve": infos[0]["iters_shift"]},
-               "dslash": dslash, "block": block, "mixed": mixed, "force": force, "roofline": roof, "roofline_dslash": roof_dslash, "cpu_baseline": cpu,
+                      "pct_of_measured": 100 * cg_gbs / peak, "equivalent_gbs": equiv_bytes_site * vh / secs / 1e9,
+                      "solves": nsolves, "iters_shift_first_solve": infos[0]["iters_shift"],
+                      "kernels": [norm_kernel(k) for k in step_kernels]},
+               "dslash": dslash, "solves_other_variants": solves, "block": block, "mixed": mixed, "force": force,
                "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
                        "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": te_s / e2e_steps,
                        "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},
                "gpu_launches": int(launches), "options": args.opt, "clocks": clk, "pack_ms": pack_ms, "input_gen_s": gen_s}
+        # free config-4 device memory before the 64^4 section
+        del packed, bdev, x, ws
+        torch.cuda.empty_cache()
+
+        # ---- config 5 (64^4) in the default run: the largest single-GPU configuration -----------------
+        c5 = None
+        if wl == "c4" and world == 1 and not args.no_c5 and prec == stag.F64 and recon == 18:
+            c5, ents = c5_section(torch, stag, args, peak, peak_src)
+            also += ents
+        out["c5"] = c5
+        roof["also"] = also
+        out["roofline"] = roof
+
+        # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            g, s_it, m = oracle_sample(cfg, U, srcs[0], 12.0)
+            cpu = {"value": g, "unit": "GFLOP/s", "cores": 1, "kind": "oracle",
+                   "sample": "%d oracle multi-shift CG iterations (maxiter=%d) of the same %d-shift solve, %.3f s/iteration"
+                             % (m, m, nshift, s_it)}
+        out["cpu_baseline"] = cpu
         print(json.dumps(out))
     if world > 1:
+        dist.barrier()
         dist.destroy_process_group()
     return 0
 
@@ -607,7 +841,9 @@ def main():
                     help="f64split = N3: fp64 vectors on split-double (b + c) links")
     ap.add_argument("--recon", type=int, default=18, choices=[18, 12])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-block", action="store_true", help="skip the N1 multi-source and N2/N3 mixed-precision measurements")
+    ap.add_argument("--no-block", action="store_true",
+                    help="skip the other storage variants' solves and the N1 multi-source, N2/N3 mixed-precision, N4 force measurements")
+    ap.add_argument("--no-c5", action="store_true", help="skip the 64^4 section of the default (c4, f64-18, 1 GPU) run")
     ap.add_argument("--ref-seconds", type=float, default=150.0,
                     help="--impl reference: total oracle time budget over all steps")
     ap.add_argument("--dslash-only", action="store_true", help="Dslash bandwidth sweep only (no CG)")

@@ -114,7 +114,14 @@ const char *stag_strerror(int err);
  * replacement — 0 never | 1, default: single-shift solves | 2 always), "cg_mixed_delta_inv" (>= 2, default 10:
  * replace the residual whenever ||r|| has fallen by this factor),
  * "cg_resident_slices" (0..3, default 3: how many of r, q, p_base the persistent kernel may keep in shared
- * memory; fewer = the global-workspace path large lattices take). */
+ * memory; fewer = the global-workspace path large lattices take),
+ * "cg_l2_keep_mb" (default 64: the persistent kernel marks the x_i, p_i of the lightest shifts — the ones that stay
+ * live longest — evict_last in L2, up to this many MB, and everything else that streams evict_first; 0: none),
+ * "cg_fill" (1, default: the persistent kernel defers the shift updates of an iteration and works them off while
+ * its CTAs wait at the sync points of the next; 0: all at once after the base shift),
+ * "cg_nbflags" (1, default: after the two stencil phases a CTA of the persistent kernel waits only for the CTAs that
+ * own its neighbouring sites; 0: for all of them),
+ * "cg_profile" (0, default; 1: see stag_cg_profile). */
 int stag_set_option(stag_ctx *ctx, const char *key, int value);
 int stag_get_option(const stag_ctx *ctx, const char *key, int *value);
 
@@ -272,6 +279,18 @@ int stag_mshift_cg_host(const stag_ctx *ctx, const void *packed, int prec, int r
                         const double *host_shifts, const double *host_residues,
                         double residue0, double stop, int maxiter, double *host_x,
                         double *host_y, void *dev_scratch, stag_cg_info *info, void *stream);
+
+/* ---- measurement aids (each roofline figure must name the kernel it is about) --------
+ * stag_kernel_log: the demangled names of the distinct kernels the calls on ctx have launched since the last
+ * stag_kernel_log_reset, one per line, into buf (host); returns their number, or STAG_ERR_BADARG if nbytes is
+ * too small.  bench.py matches these names against the kernel names of the committed ncu captures.
+ * stag_cg_profile: with option "cg_profile" = 1 the multi-kernel path of stag_mshift_cg runs without its CUDA
+ * graph and brackets each of the four kernels of iterations 8 .. 39 with CUDA events on the caller's stream;
+ * this returns the mean microseconds of a2 (D_oe), a3 (D_eo + <p,q>), a5 (r update) and a6 (shift update)
+ * launches of the last such solve and how many iterations were averaged (0: none yet). */
+int stag_kernel_log_reset(const stag_ctx *ctx);
+int stag_kernel_log(const stag_ctx *ctx, char *host_buf, size_t nbytes);
+int stag_cg_profile(const stag_ctx *ctx, double host_us_per_launch[4], int *host_iterations);
 
 #ifdef __cplusplus
 }

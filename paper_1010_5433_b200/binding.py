@@ -31,6 +31,7 @@ SYMBOLS = [
     "stag_vector_convert", "stag_cg_polish_workspace_bytes", "stag_cg_polish",
     "stag_mshift_cg_mixed_workspace_bytes", "stag_mshift_cg_mixed",
     "stag_force_workspace_bytes", "stag_fermion_force",
+    "stag_kernel_log_reset", "stag_kernel_log", "stag_cg_profile",
 ]
 
 
@@ -126,6 +127,9 @@ def lib() -> C.CDLL:
     l.stag_dslash_host.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp]
     l.stag_mshift_cg_host.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
                                       C.c_double, C.c_double, C.c_int, _vp, _vp, _vp, C.POINTER(CgInfo), _vp]
+    l.stag_kernel_log_reset.argtypes = [_vp]
+    l.stag_kernel_log.argtypes = [_vp, C.c_char_p, _sz]
+    l.stag_cg_profile.argtypes = [_vp, _dp, C.POINTER(C.c_int)]
     _lib = l
     return l
 
@@ -326,6 +330,27 @@ class Stag:
                                       _ptr(dev_force), int(bool(accumulate)), _ptr(workspace), _stream(stream))
         if rc:
             raise StagError(rc, "stag_fermion_force")
+
+    # ---- measurement aids
+    def kernel_log_reset(self):
+        lib().stag_kernel_log_reset(self._h)
+
+    def kernel_log(self) -> list:
+        """Demangled names of the distinct kernels launched on this context since kernel_log_reset()."""
+        buf = C.create_string_buffer(1 << 16)
+        rc = lib().stag_kernel_log(self._h, buf, len(buf))
+        if rc < 0:
+            raise StagError(rc, "stag_kernel_log")
+        return [n for n in buf.value.decode().split("\n") if n]
+
+    def cg_profile(self):
+        """(mean us of the a2, a3, a5, a6 launches, iterations averaged) of the last solve run with cg_profile = 1."""
+        us = (C.c_double * 4)()
+        n = C.c_int()
+        rc = lib().stag_cg_profile(self._h, us, C.byref(n))
+        if rc:
+            raise StagError(rc, "stag_cg_profile")
+        return list(us), n.value
 
     # ---- host-buffer variants
     def dslash_host(self, packed, prec, recon, out_parity, host_in, host_out, dev_scratch, stream=None):

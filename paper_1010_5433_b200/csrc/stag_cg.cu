@@ -187,15 +187,21 @@ struct CgLaunch {
 
     char *p_base() const { return ws + lay.p + (size_t)base * lay.vec_stride; }
 
-    int iteration() const {
+    // ev (nullable): 5 events recorded around the 4 launches (option cg_profile)
+    int iteration(cudaEvent_t *ev = nullptr) const {
+        if (ev) STAG_CUDA_OK(cudaEventRecord(ev[0], st));
         int rc = dslash_oe_cg_dispatch(ctx, packed, prec, recon, p_base(), ws + lay.w, state, st);
         if (rc) return rc;
+        if (ev) STAG_CUDA_OK(cudaEventRecord(ev[1], st));
         rc = dslash_eo_fused_dispatch(ctx, packed, prec, recon, ws + lay.w, p_base(), ws + lay.q,
                                       state, partials, st);
         if (rc) return rc;
-        cg_update_r_kernel<T, BLOCK><<<grid, BLOCK, 0, st>>>(nchunk, ws + lay.r, ws + lay.q, state, partials);
-        cg_update_shifts_kernel<T, BLOCK><<<grid, BLOCK, 0, st>>>(nchunk, ws + lay.r, ws + lay.p,
-                                                                 lay.vec_stride, x, x_stride, state);
+        if (ev) STAG_CUDA_OK(cudaEventRecord(ev[2], st));
+        STAG_LAUNCH_K(ctx, (cg_update_r_kernel<T, BLOCK>), grid, BLOCK, 0, st, nchunk, ws + lay.r, ws + lay.q, state, partials);
+        if (ev) STAG_CUDA_OK(cudaEventRecord(ev[3], st));
+        STAG_LAUNCH_K(ctx, (cg_update_shifts_kernel<T, BLOCK>), grid, BLOCK, 0, st, nchunk, ws + lay.r, ws + lay.p,
+                      lay.vec_stride, x, x_stride, state);
+        if (ev) STAG_CUDA_OK(cudaEventRecord(ev[4], st));
         STAG_CUDA_OK(cudaGetLastError());
         return STAG_OK;
     }
@@ -209,16 +215,28 @@ static int run_multikernel(const CgLaunch<T> &L, const void *b, void *y, int max
     typedef CgLaunch<T> Lz;
     const stag_ctx *ctx = L.ctx;
     cudaStream_t st = L.st;
-    cg_init_kernel<T, Lz::BLOCK><<<L.grid, Lz::BLOCK, 0, st>>>(
-        L.nchunk, static_cast<const char *>(b), L.ws + L.lay.r, L.ws + L.lay.p, L.lay.vec_stride, L.x,
-        L.x_stride, L.state, L.partials);
+    STAG_LAUNCH_K(ctx, (cg_init_kernel<T, Lz::BLOCK>), L.grid, Lz::BLOCK, 0, st, L.nchunk, static_cast<const char *>(b),
+                  L.ws + L.lay.r, L.ws + L.lay.p, L.lay.vec_stride, L.x, L.x_stride, L.state, L.partials);
     STAG_CUDA_OK(cudaGetLastError());
 
     // iterations in batches of cg_check_every; one batch always in flight behind the one polled
     const int batch = ctx->opt.cg_check_every;
     cudaGraphExec_t gexec = nullptr;
     int rc = STAG_OK;
-    if (ctx->opt.cg_graph && maxiter > 0) {
+    // option cg_profile (measurement aid, stag_cg_profile): no graph; CUDA events around each of the four kernels
+    // of iterations kProfSkip .. kProfSkip + kProfIters - 1, averaged per kernel after the solve
+    constexpr int kProfSkip = 8, kProfIters = 32;
+    const bool profile = ctx->opt.cg_profile != 0;
+    cudaEvent_t pev[kProfIters][5];
+    int nprof = 0;
+    if (profile) {
+        ctx->prof_iters = 0;
+        for (int i = 0; i < kProfIters && rc == STAG_OK; ++i)
+            for (int j = 0; j < 5; ++j)
+                if (cudaEventCreate(&pev[i][j]) != cudaSuccess) rc = STAG_ERR_CUDA;
+        if (rc) { cudaGetLastError(); return rc; }
+    }
+    if (ctx->opt.cg_graph && maxiter > 0 && !profile) {
         cudaGraph_t graph = nullptr;
         cudaStream_t cap = nullptr;
         // capture on a private stream so the caller's stream (possibly the legacy default) is untouched
@@ -246,7 +264,12 @@ static int run_multikernel(const CgLaunch<T> &L, const void *b, void *y, int max
             if (gexec) {
                 if (cudaGraphLaunch(gexec, st) != cudaSuccess) rc = STAG_ERR_CUDA;
             } else {
-                for (int j = 0; j < batch && rc == STAG_OK; ++j) rc = L.iteration();
+                for (int j = 0; j < batch && rc == STAG_OK; ++j) {
+                    const int it = k * batch + j;
+                    const bool rec = profile && it >= kProfSkip && nprof < kProfIters;
+                    rc = L.iteration(rec ? pev[nprof] : nullptr);
+                    nprof += rec;
+                }
             }
             if (rc == STAG_OK &&
                 (cudaMemcpyAsync((void *)(poll + (k & 1)), &L.state->done, sizeof(int),
@@ -262,12 +285,27 @@ static int run_multikernel(const CgLaunch<T> &L, const void *b, void *y, int max
     if (ev[0]) cudaEventDestroy(ev[0]);
     if (ev[1]) cudaEventDestroy(ev[1]);
     if (gexec) cudaGraphExecDestroy(gexec);
+    if (profile) {
+        double sum[4] = {0.0, 0.0, 0.0, 0.0};
+        if (rc == STAG_OK && nprof > 0 && cudaEventSynchronize(pev[nprof - 1][4]) == cudaSuccess) {
+            for (int i = 0; i < nprof; ++i)
+                for (int j = 0; j < 4; ++j) {
+                    float ms = 0.f;
+                    cudaEventElapsedTime(&ms, pev[i][j], pev[i][j + 1]);
+                    sum[j] += ms * 1e3;
+                }
+            for (int j = 0; j < 4; ++j) ctx->prof_us[j] = sum[j] / nprof;
+            ctx->prof_iters = nprof;        // (iterations run after the latch closed would count as ~0: stop is far here)
+        }
+        for (int i = 0; i < kProfIters; ++i)
+            for (int j = 0; j < 5; ++j) cudaEventDestroy(pev[i][j]);
+    }
     if (rc) { cudaGetLastError(); return rc; }
 
     if (y) {
         ++launches;
-        cg_partial_fraction_kernel<T, Lz::BLOCK><<<L.grid, Lz::BLOCK, 0, st>>>(
-            L.nchunk, static_cast<const char *>(b), L.x, L.x_stride, static_cast<char *>(y), L.state);
+        STAG_LAUNCH_K(ctx, (cg_partial_fraction_kernel<T, Lz::BLOCK>), L.grid, Lz::BLOCK, 0, st, L.nchunk,
+                      static_cast<const char *>(b), L.x, L.x_stride, static_cast<char *>(y), L.state);
         STAG_CUDA_OK(cudaGetLastError());
     }
     *launches_out = launches;

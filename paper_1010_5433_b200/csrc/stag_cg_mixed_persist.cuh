@@ -376,6 +376,7 @@ int launch_mixed(const stag_ctx *ctx, const MixedArgs &args, cudaStream_t st) {
     if (per_sm < 1) return STAG_ERR_UNSUPPORTED;
     Geom gg = g;
     void *params[] = {(void *)&gg, (void *)&a};
+    log_kernel(ctx, (const void *)kern);
     STAG_CUDA_OK(cudaLaunchCooperativeKernel((const void *)kern, dim3(grid), dim3(NT), params, smem, st));
     return STAG_OK;
 }

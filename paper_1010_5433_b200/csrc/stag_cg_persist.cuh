@@ -829,6 +829,7 @@ int launch_persistent(const stag_ctx *ctx, const PersistArgs &args, cudaStream_t
     STAG_CUDA_OK(cudaMemsetAsync(a.flags, 0, (size_t)grid * 128, st));
     Geom gg = g;
     void *params[] = {(void *)&gg, (void *)&a};
+    log_kernel(ctx, (const void *)kern);
     STAG_CUDA_OK(cudaLaunchCooperativeKernel((const void *)kern, dim3(grid), dim3(NT), params, smem, st));
     return STAG_OK;
 }

@@ -69,6 +69,7 @@ struct Options {
     int cg_l2_keep_mb;       // persistent kernel: MB of x_i, p_i (lightest shifts first) kept L2-resident (evict_last); 0: none
     int cg_fill;             // persistent kernel: 1 = deferred shift updates are worked off while waiting at sync points
     int cg_nbflags;          // persistent kernel: 1 = neighbour epoch flags instead of grid barriers after phases A and D
+    int cg_profile;          // multi-kernel path: 1 = no graph, CUDA events around every kernel of 32 iterations (stag_cg_profile)
 };
 
 }  // namespace stag
@@ -80,6 +81,12 @@ struct stag_ctx {
     int num_sms;
     int *pinned_flags;   // 512 B pinned (mapped) host buffer: status words, convergence polls; bytes 128.. = 16 doubles (N2 norms)
     void *pinned_info;   // pinned staging for the CG state upload / read-back (one CgState)
+    // measurement aids (stag_kernel_log, stag_cg_profile): which kernels the calls on this ctx launched, and the
+    // per-kernel times of the last profiled multi-kernel solve
+    mutable const void *klog[32];
+    mutable int nklog;
+    mutable double prof_us[4];
+    mutable int prof_iters;
 };
 
 namespace stag {
@@ -88,6 +95,20 @@ namespace stag {
     do {                                                    \
         cudaError_t e__ = (call);                           \
         if (e__ != cudaSuccess) return STAG_ERR_CUDA;       \
+    } while (0)
+
+// remember that `func` (a __global__ function) was launched on behalf of ctx (stag_kernel_log)
+inline void log_kernel(const stag_ctx *ctx, const void *func) {
+    for (int i = 0; i < ctx->nklog; ++i)
+        if (ctx->klog[i] == func) return;
+    if (ctx->nklog < 32) ctx->klog[ctx->nklog++] = func;
+}
+// launch kern<<<...>>>(args) and log it; `kern` is an expression of function-pointer type
+#define STAG_LAUNCH_K(ctx, kern, grid, block, smem, st, ...)             \
+    do {                                                                  \
+        auto k__ = kern;                                                  \
+        stag::log_kernel(ctx, reinterpret_cast<const void *>(k__));       \
+        k__<<<grid, block, smem, st>>>(__VA_ARGS__);                      \
     } while (0)
 
 inline bool valid_prec(int p) { return p == STAG_F64 || p == STAG_F32 || p == STAG_F64_SPLIT; }

@@ -1,6 +1,9 @@
 // stag_ctx.cu — context, options, sizes, error strings of libstag_b200.so.
+#include <cstdlib>
 #include <cstring>
+#include <cxxabi.h>
 #include <new>
+#include <string>
 
 #include "stag_cg.cuh"
 
@@ -91,6 +94,7 @@ static int *option_slot(Options &o, const char *key) {
     if (!std::strcmp(key, "cg_l2_keep_mb")) return &o.cg_l2_keep_mb;
     if (!std::strcmp(key, "cg_fill")) return &o.cg_fill;
     if (!std::strcmp(key, "cg_nbflags")) return &o.cg_nbflags;
+    if (!std::strcmp(key, "cg_profile")) return &o.cg_profile;
     return nullptr;
 }
 
@@ -109,7 +113,8 @@ extern "C" int stag_set_option(stag_ctx *ctx, const char *key, int value) {
     if (slot == &ctx->opt.cg_resident_slices && (value < 0 || value > 3)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_ctas_per_sm && (value < 1 || value > 16)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_l2_keep_mb && (value < 0 || value > 1024)) return STAG_ERR_BADARG;
-    if ((slot == &ctx->opt.cg_fill || slot == &ctx->opt.cg_nbflags) && (value < 0 || value > 1)) return STAG_ERR_BADARG;
+    if ((slot == &ctx->opt.cg_fill || slot == &ctx->opt.cg_nbflags || slot == &ctx->opt.cg_profile) &&
+        (value < 0 || value > 1)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.dslash_ctas_per_sm && (value < 0 || value > 32)) return STAG_ERR_BADARG;
     *slot = value;
     return STAG_OK;
@@ -150,4 +155,35 @@ extern "C" size_t stag_host_scratch_bytes(const stag_ctx *ctx, int prec, int nsh
     // canonical staging, b, y, x[nshift], CG workspace
     return canon + 2 * vec + align256((size_t)nshift * stag_vector_bytes(ctx, prec)) +
            align256(cg_workspace_layout(ctx, prec, nshift, nullptr));
+}
+
+// ---- measurement aids -------------------------------------------------------------------------------
+extern "C" int stag_kernel_log_reset(const stag_ctx *ctx) {
+    if (!ctx) return STAG_ERR_BADARG;
+    ctx->nklog = 0;
+    return STAG_OK;
+}
+
+extern "C" int stag_kernel_log(const stag_ctx *ctx, char *buf, size_t nbytes) {
+    if (!ctx || !buf || nbytes == 0) return STAG_ERR_BADARG;
+    std::string out;
+    for (int i = 0; i < ctx->nklog; ++i) {
+        const char *mangled = nullptr;
+        if (cudaFuncGetName(&mangled, ctx->klog[i]) != cudaSuccess || !mangled) { cudaGetLastError(); continue; }
+        int status = 0;
+        char *dem = abi::__cxa_demangle(mangled, nullptr, nullptr, &status);
+        out += (status == 0 && dem) ? dem : mangled;
+        out += '\n';
+        std::free(dem);
+    }
+    if (out.size() + 1 > nbytes) return STAG_ERR_BADARG;
+    std::memcpy(buf, out.c_str(), out.size() + 1);
+    return ctx->nklog;
+}
+
+extern "C" int stag_cg_profile(const stag_ctx *ctx, double us_per_launch[4], int *iterations) {
+    if (!ctx || !us_per_launch || !iterations) return STAG_ERR_BADARG;
+    for (int j = 0; j < 4; ++j) us_per_launch[j] = ctx->prof_us[j];
+    *iterations = ctx->prof_iters;
+    return STAG_OK;
 }

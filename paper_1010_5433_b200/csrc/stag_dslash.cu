@@ -86,8 +86,8 @@ static int launch_dslash_block(const stag_ctx *ctx, const void *packed, const vo
     // registers: R accumulators + one matrix + one neighbour.  fp64: 128 per thread up to R = 2, 255 at
     // R = 4 (24 fp64 accumulators alone are 48 registers); fp32: 64 / 128.
     constexpr int RT = sizeof(T) == 8 ? (R >= 4 ? 256 : 512) : (R >= 2 ? 512 : 1024);
-    dslash_block_kernel<T, RECON, BLOCK, RT, R><<<grid, BLOCK, 0, st>>>(
-        g, W, static_cast<const char *>(in), static_cast<char *>(out), par, stride, nrhs);
+    STAG_LAUNCH_K(ctx, (dslash_block_kernel<T, RECON, BLOCK, RT, R>), grid, BLOCK, 0, st, g, W,
+                  static_cast<const char *>(in), static_cast<char *>(out), par, stride, nrhs);
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
 }
@@ -127,9 +127,9 @@ static int launch_dslash(const stag_ctx *ctx, const void *packed, const void *in
     if (regs == 0) regs = sizeof(T) == 8 ? 128 : 64;
     if (regs == 64 && sizeof(T) == 8 && RECON == 12) regs = 128;
 #define STAG_LAUNCH(B)                                                                                            \
-    if (regs == 64) dslash_kernel<T, RECON, B, MODE, 1024><<<grid, B, 0, st>>>(g, W, i, o, par, pp, state, partials);      \
-    else if (regs == 128) dslash_kernel<T, RECON, B, MODE, 512><<<grid, B, 0, st>>>(g, W, i, o, par, pp, state, partials); \
-    else dslash_kernel<T, RECON, B, MODE, 256><<<grid, B, 0, st>>>(g, W, i, o, par, pp, state, partials)
+    if (regs == 64) STAG_LAUNCH_K(ctx, (dslash_kernel<T, RECON, B, MODE, 1024>), grid, B, 0, st, g, W, i, o, par, pp, state, partials);      \
+    else if (regs == 128) STAG_LAUNCH_K(ctx, (dslash_kernel<T, RECON, B, MODE, 512>), grid, B, 0, st, g, W, i, o, par, pp, state, partials); \
+    else STAG_LAUNCH_K(ctx, (dslash_kernel<T, RECON, B, MODE, 256>), grid, B, 0, st, g, W, i, o, par, pp, state, partials)
     switch (block) {
         case 64: STAG_LAUNCH(64); break;
         case 256: STAG_LAUNCH(256); break;
@@ -146,9 +146,9 @@ static int launch_dslash_split(const stag_ctx *ctx, const void *packed, const vo
                                const void *p, CgState *state, double *partials, cudaStream_t st) {
     const Geom &g = ctx->g;
     const int grid = dslash_grid(ctx, 128, MODE == 2);
-    dslash_kernel<double, RECON, 128, MODE, 512, true><<<grid, 128, 0, st>>>(
-        g, static_cast<const char *>(packed), static_cast<const char *>(in), static_cast<char *>(out), par,
-        static_cast<const char *>(p), state, partials);
+    STAG_LAUNCH_K(ctx, (dslash_kernel<double, RECON, 128, MODE, 512, true>), grid, 128, 0, st, g,
+                  static_cast<const char *>(packed), static_cast<const char *>(in), static_cast<char *>(out), par,
+                  static_cast<const char *>(p), state, partials);
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
 }

@@ -47,8 +47,8 @@ static int launch_pipe(const stag_ctx *ctx, const void *packed, const void *in, 
         if (cap < grid) grid = cap;
     }
     const size_t stride = (size_t)g.Vh * 6 * sizeof(T);
-    kern<<<grid, BLOCK, smem, st>>>(g, static_cast<const char *>(packed), static_cast<const char *>(in),
-                                    static_cast<char *>(out), par, stride, nrhs);
+    STAG_LAUNCH_K(ctx, kern, grid, BLOCK, smem, st, g, static_cast<const char *>(packed), static_cast<const char *>(in),
+                  static_cast<char *>(out), par, stride, nrhs);
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
 }

@@ -160,7 +160,7 @@ extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int p
     const char *W = static_cast<const char *>(packed);
     // occupancy / unroll measured at 32^3 x 8, 16 shifts (profiles/README.md "N4"): fp64 is fastest with 128
     // registers (16 warps per SM) and the shift loop unrolled x2, fp32 with 3 CTAs per SM and x4
-#define STAG_FORCE(T, R, M, U) force_kernel<T, R, M, U><<<grid, block, 0, st>>>(g, W, x, w, vbytes, nshift, coef, dev_force, accumulate)
+#define STAG_FORCE(T, R, M, U) STAG_LAUNCH_K(ctx, (force_kernel<T, R, M, U>), grid, block, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate)
     if (prec == STAG_F64) { if (recon == 18) STAG_FORCE(double, 18, 4, 2); else STAG_FORCE(double, 12, 4, 2); }
     else { if (recon == 18) STAG_FORCE(float, 18, 3, 4); else STAG_FORCE(float, 12, 3, 4); }
 #undef STAG_FORCE

@@ -125,8 +125,9 @@ static int polish(const stag_ctx *ctx, const void *packed, int prec, int recon, 
     int launches = 0;
 
     STAG_CUDA_OK(cudaMemsetAsync(ws + lay.scal, 0, 256, st));
-    defect_kernel<256><<<grid, 256, 0, st>>>(nchunk, reinterpret_cast<const double2 *>(b), nullptr, nullptr, 0.0,
-                                              nullptr, partials, ticket, scal + 7);
+    STAG_LAUNCH_K(ctx, defect_kernel<256>, grid, 256, 0, st, nchunk, reinterpret_cast<const double2 *>(b),
+                  static_cast<const double2 *>(nullptr), static_cast<const double2 *>(nullptr), 0.0,
+                  static_cast<double2 *>(nullptr), partials, ticket, scal + 7);
     ++launches;
     STAG_CUDA_OK(cudaMemcpyAsync((void *)hn, scal, 8 * sizeof(double), cudaMemcpyDeviceToHost, st));
     STAG_CUDA_OK(cudaStreamSynchronize(st));
@@ -142,7 +143,7 @@ static int polish(const stag_ctx *ctx, const void *packed, int prec, int recon, 
         rc = dslash_n(ctx, packed, prec, recon, 0, n, ws + lay.w, ws + lay.e, vbytes, st, &launches);   // e as scratch
         if (rc) return rc;
         for (int s = 0; s < n; ++s) {
-            defect_kernel<256><<<grid, 256, 0, st>>>(
+            STAG_LAUNCH_K(ctx, defect_kernel<256>, grid, 256, 0, st,
                 nchunk, reinterpret_cast<const double2 *>(b), reinterpret_cast<const double2 *>(xg + s * vbytes),
                 reinterpret_cast<const double2 *>(ws + lay.e + s * vbytes), mass * mass + shifts[i0 + s],
                 reinterpret_cast<double2 *>(ws + lay.r + s * vbytes), partials, ticket, scal + s);
