@@ -174,9 +174,10 @@ int stag_mshift_cg(const stag_ctx *ctx, const void *packed, int prec, int recon,
                    void *x_even, void *y_even, void *workspace, stag_cg_info *info,
                    void *stream);
 
-/* ---- N1: the hopping term on nrhs (1 .. STAG_MAX_RHS) independent vectors with
- * ONE read of the links.  in / out: nrhs contiguous device-format vectors (stride
- * stag_vector_bytes); out_parity 0 = D_eo (even output, odd input), 1 = D_oe.  One launch, no sync. */
+/* ---- N1: the hopping term on nrhs independent vectors, STAG_MAX_RHS of them per read of
+ * the links.  in / out: nrhs (1 .. STAG_MAX_SHIFTS) contiguous device-format vectors (stride
+ * stag_vector_bytes); out_parity 0 = D_eo (even output, odd input), 1 = D_oe.  nrhs <= STAG_MAX_RHS: one launch;
+ * more: groups of STAG_MAX_RHS, in one launch where the cp.async-ring kernel applies.  No sync. */
 int stag_dslash_block(const stag_ctx *ctx, const void *packed, int prec, int recon, int out_parity,
                       int nrhs, const void *in, void *out, void *stream);
 
@@ -262,7 +263,7 @@ int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, int prec_hi
  *              accumulate != 0 adds to it (several pseudo-fermions)
  *   workspace  stag_force_workspace_bytes (the nshift odd vectors D_oe x_i), 256-byte aligned
  * prec = STAG_F64 | STAG_F32 (the paper's choice for the force); outer products in prec, the
- * 3x3 product and projection in fp64.  Asynchronous: 1 + ceil(nshift / STAG_MAX_RHS) launches, no sync. */
+ * 3x3 product and projection in fp64.  Asynchronous: 2 launches (all D_oe x_i, then the force), no sync. */
 size_t stag_force_workspace_bytes(const stag_ctx *ctx, int prec, int nshift);
 int stag_fermion_force(const stag_ctx *ctx, const void *packed, int prec, int recon, int nshift,
                        const double *host_residues, const void *x_even, double *dev_force, int accumulate,

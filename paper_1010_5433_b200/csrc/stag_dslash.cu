@@ -199,12 +199,22 @@ extern "C" int stag_dslash_block(const stag_ctx *ctx, const void *packed, int pr
     using namespace stag;
     if (!ctx || !packed || !in || !out || in == out) return STAG_ERR_BADARG;
     if (!valid_prec(prec) || !valid_recon(recon) || (out_parity != 0 && out_parity != 1)) return STAG_ERR_BADARG;
-    if (nrhs < 1 || nrhs > STAG_MAX_RHS) return STAG_ERR_BADARG;
+    if (nrhs < 1 || nrhs > STAG_MAX_SHIFTS) return STAG_ERR_BADARG;
     if (prec == STAG_F64_SPLIT) return STAG_ERR_UNSUPPORTED;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (ctx->opt.dslash_pipe != 0) {
         const int rc = dslash_pipe_dispatch(ctx, packed, prec, recon, out_parity, nrhs, in, out, st);
         if (rc != STAG_ERR_UNSUPPORTED) return rc;
+    }
+    if (nrhs > STAG_MAX_RHS) {                       // groups of STAG_MAX_RHS, one launch each
+        const size_t vb = (size_t)ctx->g.Vh * vec_bytes_per_site(prec);
+        for (int i0 = 0; i0 < nrhs; i0 += STAG_MAX_RHS) {
+            const int n = nrhs - i0 < STAG_MAX_RHS ? nrhs - i0 : STAG_MAX_RHS;
+            const int rc = stag_dslash_block(ctx, packed, prec, recon, out_parity, n, static_cast<const char *>(in) + i0 * vb,
+                                             static_cast<char *>(out) + i0 * vb, stream);
+            if (rc) return rc;
+        }
+        return STAG_OK;
     }
     if (prec == STAG_F64)
         return recon == 18 ? dslash_block_r<double, 18>(ctx, packed, in, out, out_parity, nrhs, st)

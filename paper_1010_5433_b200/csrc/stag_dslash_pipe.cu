@@ -16,9 +16,14 @@ constexpr int pipe_ctas_per_sm() {
 
 template <typename T, int RECON, int R, int BLOCK, int STAGES, bool VA>
 __global__ void __launch_bounds__(BLOCK, (pipe_ctas_per_sm<T, RECON, R, BLOCK, STAGES, VA>()))
-dslash_pipe_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ in,
-                   char *__restrict__ out, const int par, const size_t stride, const int nrhs) {
+dslash_pipe_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ in_all,
+                   char *__restrict__ out_all, const int par, const size_t stride, const int nvec) {
     extern __shared__ __align__(16) unsigned char ring[];
+    // blockIdx.y = group of R vectors (stag_fermion_force: the D_oe x_i of all shifts in ONE launch, so that the
+    // groups' fill / drain ramps overlap); the last group may be short
+    const char *in = in_all + (size_t)blockIdx.y * R * stride;
+    char *out = out_all + (size_t)blockIdx.y * R * stride;
+    const int left = nvec - (int)blockIdx.y * R, nrhs = left < R ? left : R;
     const char *ins[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) ins[r] = in + (size_t)(r < nrhs ? r : 0) * stride;
@@ -33,7 +38,7 @@ dslash_pipe_kernel(const Geom g, const char *__restrict__ W, const char *__restr
 }
 
 template <typename T, int RECON, int R, int BLOCK, int STAGES, bool VA>
-static int launch_pipe(const stag_ctx *ctx, const void *packed, const void *in, void *out, int par, int nrhs,
+static int launch_pipe(const stag_ctx *ctx, const void *packed, const void *in, void *out, int par, int nvec,
                        cudaStream_t st) {
     const Geom &g = ctx->g;
     constexpr int smem = STAGES * pipe_stage_bytes<T, RECON, R, BLOCK, VA>();
@@ -47,8 +52,8 @@ static int launch_pipe(const stag_ctx *ctx, const void *packed, const void *in, 
         if (cap < grid) grid = cap;
     }
     const size_t stride = (size_t)g.Vh * 6 * sizeof(T);
-    STAG_LAUNCH_K(ctx, kern, grid, BLOCK, smem, st, g, static_cast<const char *>(packed), static_cast<const char *>(in),
-                  static_cast<char *>(out), par, stride, nrhs);
+    STAG_LAUNCH_K(ctx, kern, dim3(grid, (nvec + R - 1) / R), BLOCK, smem, st, g, static_cast<const char *>(packed),
+                  static_cast<const char *>(in), static_cast<char *>(out), par, stride, nvec);
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
 }
@@ -60,6 +65,7 @@ static int launch_pipe(const stag_ctx *ctx, const void *packed, const void *in, 
 template <typename T, int RECON>
 static int pipe_r(const stag_ctx *ctx, const void *packed, const void *in, void *out, int par, int nrhs,
                   cudaStream_t st) {
+    // nrhs > 4: groups of four in one launch (blockIdx.y)
     if (sizeof(T) == 8) {
         if (nrhs <= 2) return STAG_ERR_UNSUPPORTED;               // register-staged kernel is as fast
         return launch_pipe<T, RECON, 4, 128, 2, true>(ctx, packed, in, out, par, nrhs, st);

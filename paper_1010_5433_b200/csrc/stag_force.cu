@@ -147,11 +147,10 @@ extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int p
     const size_t vbytes = (size_t)g.Vh * vec_bytes_per_site(prec);
     const char *x = static_cast<const char *>(x_even);
     char *w = static_cast<char *>(workspace);
-    // w_i = D_oe x_i, STAG_MAX_RHS shifts per read of the links (N1 kernel)
-    for (int i0 = 0; i0 < nshift; i0 += STAG_MAX_RHS) {
-        const int n = nshift - i0 < STAG_MAX_RHS ? nshift - i0 : STAG_MAX_RHS;
-        const int rc = stag_dslash_block(ctx, packed, prec, recon, 1, n, x + (size_t)i0 * vbytes,
-                                         w + (size_t)i0 * vbytes, st);
+    // w_i = D_oe x_i, STAG_MAX_RHS shifts per read of the links (N1 kernel); all groups of four in ONE launch of
+    // the cp.async-ring kernel where it applies, so that the groups' fill / drain ramps overlap
+    {
+        const int rc = stag_dslash_block(ctx, packed, prec, recon, 1, nshift, x, w, st);
         if (rc) return rc;
     }
     ForceCoef coef;

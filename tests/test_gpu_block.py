@@ -154,11 +154,32 @@ def test_block_badargs(stag):
     packed = ctx.upload_gauge(si.links_unit(L), 0, 18)
     v = ctx.alloc(5 * ctx.vector_bytes(0))
     w = ctx.alloc(5 * ctx.vector_bytes(0))
-    for nrhs in (0, 5):
+    for nrhs in (0, stag.MAX_SHIFTS + 1):
         with pytest.raises(stag.StagError) as ei:
             ctx.dslash_block(packed, 0, 18, 0, nrhs, v, w)
         assert ei.value.code == stag.ERR_BADARG
     assert ctx.cg_block_workspace_bytes(0, 4, 5) == 0
+
+
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (16, 16, 16, 4), (6, 4, 2, 8)])
+@pytest.mark.parametrize("prec,recon", [(0, 18), (1, 12)])
+@pytest.mark.parametrize("nvec", [5, 8, 11])
+@pytest.mark.parametrize("pipe", [1, 0])
+def test_dslash_block_more_vectors_than_one_link_read_serves(stag, L, prec, recon, nvec, pipe):
+    """nrhs > STAG_MAX_RHS: groups of four per read of the links — ONE launch (grid.y = group) where the
+    cp.async-ring kernel applies (what stag_fermion_force uses for the D_oe x_i of all its shifts), one launch per
+    group otherwise; a short last group included.  Every vector against the oracle."""
+    U = si.links_haar(L, 23)
+    ctx = stag.Stag(L)
+    ctx.set_option("dslash_pipe", pipe)
+    packed = ctx.upload_gauge(U, prec, recon)
+    vb = ctx.vector_bytes(prec)
+    vs = [si.source_gaussian(L, 23, stream=1 + k) for k in range(nvec)]
+    vin, vout = ctx.upload_vectors(vs, prec), ctx.alloc(nvec * vb)
+    vout.fill_(0xFF)
+    ctx.dslash_block(packed, prec, recon, 1, nvec, vin, vout)
+    for k in range(nvec):
+        assert rel(ctx.download_vector(vout, prec, k * vb), oracle.dslash(L, U, vs[k], 1)) <= TOL[prec]
 
 
 @pytest.mark.parametrize("slices", [0, 1, 2, 3])
