@@ -462,8 +462,10 @@ def measure_block(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak
 
 
 def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
-    """N2 + N3: stag_mshift_cg_mixed on ONE resident split-double buffer (fp32 stage reads its b planes, the
-    fp64 polish reads b + c), same source, shifts and stop as the fp64 step; second of two runs timed."""
+    """N2 + N3: stag_mshift_cg_mixed with DEFAULT options on ONE resident split-double buffer (fp32 reads its b planes,
+    fp64 reads b + c) against stag_mshift_cg in fp64 on native fp64 links, for the lightest 1, 2, 4, 8, 16 shifts of
+    the workload, same source and stop; the call picks its route (1 residual replacement | 2 fp32 + polish | 3 fp64
+    multi-shift).  Then the fp32 + polish route forced at all 16 shifts, for the record."""
     n = len(cfg["shifts"])
     split = ctx.upload_gauge(U, stag.F64_SPLIT, 18)
     p64 = ctx.upload_gauge(U, stag.F64, 18)
@@ -471,28 +473,27 @@ def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
     b = ctx.upload_vector(srcs[0], stag.F64)
     x = ctx.alloc(n * vb)
     ws = ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(n))
-    out = {}
-    for name, hi, prec_hi, lo in (("split_buffer", split, stag.F64_SPLIT, split), ("f64_polish_f32_inner", p64, stag.F64, split)):
-        secs, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(hi, prec_hi, 18, lo, 18, b, cfg["mass"], cfg["shifts"],
-                                                                         cfg["stops"][0], 100000, x, ws))
-        out[name] = {"rc": rc, "s_per_solve": secs, "vs_fp64_multishift": fp64_s_per_solve / secs,
-                     "inner_fp32_iters": info["inner"]["iters"], "polish_iters": info["polish"]["iters"],
-                     "polish_passes": info["polish"]["passes"],
-                     "true_resid_after_fp32": max(info["polish"]["resid_before"]),
-                     "true_resid_final": max(info["polish"]["resid_after"]),
-                     "kernel_launches": info["inner"]["kernel_launches"] + info["polish"]["kernel_launches"]}
-    # single shift (the lightest): the inner stage is the persistent residual-replacement kernel and stops on the
-    # TRUE fp64 residual, nothing is left to polish; the fp64 solver on the same single system beside it
-    sh1 = cfg["shifts"][:1]
-    cgws = ctx.alloc(ctx.cg_workspace_bytes(stag.F64, 1))
-    t64, (rc64, i64) = timed_call(torch, lambda: ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], sh1, cfg["stops"][0], 100000, x, cgws))
-    # fp32 iterations on the b planes, fp64 residual replacement on b + c of the SAME split-double buffer (N3)
-    tm, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], sh1,
-                                                                   cfg["stops"][0], 100000, x, ws))
-    out["single_shift_residual_replacement"] = {
-        "rc": rc, "s_per_solve": tm, "fp64_s_per_solve": t64, "vs_fp64": t64 / tm, "iters": info["inner"]["iters"],
-        "fp64_iters": i64["iters"], "reliable_updates": info["reliable_updates"],
-        "polish_iters": sum(info["polish"]["iters"]), "true_resid_final": info["polish"]["resid_after"][0]}
+    cgws = ctx.alloc(ctx.cg_workspace_bytes(stag.F64, n))
+    out = {"by_nshift": {}}
+    for k in sorted({1, 2, 4, 8, n} & set(range(1, n + 1))):
+        sh = cfg["shifts"][:k]
+        t64, (rc64, i64) = timed_call(torch, lambda: ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], sh, cfg["stops"][0], 100000, x, cgws))
+        tm, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], sh,
+                                                                       cfg["stops"][0], 100000, x, ws))
+        out["by_nshift"][str(k)] = {
+            "rc": rc, "route": info["route"], "s_per_solve": tm, "fp64_s_per_solve": t64, "vs_fp64_multishift": t64 / tm,
+            "inner_iters": info["inner"]["iters"], "fp64_iters": i64["iters"], "reliable_updates": info["reliable_updates"],
+            "polish_iters": sum(info["polish"]["iters"]), "true_resid_final": max(info["polish"]["resid_after"])}
+    ctx.set_option("cg_mixed_fp64_from", 0)
+    secs, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], cfg["shifts"],
+                                                                     cfg["stops"][0], 100000, x, ws))
+    ctx.set_option("cg_mixed_fp64_from", 3)
+    out["forced_fp32_plus_polish_all_shifts"] = {
+        "rc": rc, "route": info["route"], "s_per_solve": secs, "vs_fp64_multishift": fp64_s_per_solve / secs,
+        "inner_fp32_iters": info["inner"]["iters"], "polish_iters": sum(info["polish"]["iters"]),
+        "polish_passes": info["polish"]["passes"], "true_resid_after_fp32": max(info["polish"]["resid_before"]),
+        "true_resid_final": max(info["polish"]["resid_after"]),
+        "kernel_launches": info["inner"]["kernel_launches"] + info["polish"]["kernel_launches"]}
     return out
 
 

@@ -110,6 +110,8 @@ const char *stag_strerror(int err);
  * "cg_persistent" (1, default: lattices whose r, q, p_base slices fit in shared memory run the
  * whole solve as one cooperative kernel; 0: always the multi-kernel path),
  * "cg_persistent_threads" (0 auto | 256 | 512 | 1024 threads per CTA of that kernel),
+ * "cg_mixed_fp64_from" (default 3; stag_mshift_cg_mixed runs the fp64 multi-shift solve from this many shifts on,
+ * 0: never),
  * "cg_mixed_reliable" (stag_mshift_cg_mixed: run the inner stage as the persistent kernel with residual
  * replacement — 0 never | 1, default: single-shift solves | 2 always), "cg_mixed_delta_inv" (>= 2, default 10:
  * replace the residual whenever ||r|| has fallen by this factor),
@@ -218,9 +220,10 @@ typedef struct stag_polish_info {
     int kernel_launches;
 } stag_polish_info;
 typedef struct stag_mixed_info {
-    stag_cg_info inner;                      /* the inner (fp32-matrix) multi-shift run                   */
+    stag_cg_info inner;                      /* the inner multi-shift run (fp32 matrices; route 3: fp64)  */
     stag_polish_info polish;
     int reliable_updates;                    /* residual replacements of the inner run (0: plain fp32 run) */
+    int route;                               /* 1 residual replacement | 2 fp32 + polish | 3 fp64 multi-shift */
 } stag_mixed_info;
 
 /* dst = src converted between device vector formats (nvec contiguous vectors each side). */
@@ -236,7 +239,11 @@ int stag_cg_polish(const stag_ctx *ctx, const void *packed, int prec, int recon,
                    double mass, int nshift, const double *host_shifts, double stop, int maxiter,
                    void *x_even, void *workspace, stag_polish_info *info, void *stream);
 
-/* Inner stage, then the polish, then y.  Inner stage, single shift with recon_hi =
+/* Inner stage, then the polish, then y.  The call picks the fastest route to the fp64 stop for the number of
+ * shifts (info->route; option "cg_mixed_fp64_from", default 3): from that many shifts on — where the per-shift polish
+ * costs more than fp32 saved — it IS the fp64 multi-shift solve on packed_hi (the paper's own choice for the
+ * Metropolis solves), followed by the same true-residual check; with stop >= 1e-6, which fp32 can
+ * reach, always the fp32 routes.  Inner stage, single shift with recon_hi =
  * recon_lo (option "cg_mixed_reliable"): ONE persistent kernel with RESIDUAL REPLACEMENT (ref [7]):
  * fp32 matrices, r, q, p; x in fp64; whenever ||r|| has fallen tenfold, and again at stop, the true residual
  * b - (A + sigma) x is recomputed with the fp64 matrices and replaces the recursive one; convergence is declared

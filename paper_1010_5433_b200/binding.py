@@ -59,11 +59,11 @@ class PolishInfo(C.Structure):
 
 
 class MixedInfo(C.Structure):
-    _fields_ = [("inner", CgInfo), ("polish", PolishInfo), ("reliable_updates", C.c_int)]
+    _fields_ = [("inner", CgInfo), ("polish", PolishInfo), ("reliable_updates", C.c_int), ("route", C.c_int)]
 
     def as_dict(self, nshift: int) -> dict:
         return dict(inner=self.inner.as_dict(nshift), polish=self.polish.as_dict(nshift),
-                    reliable_updates=self.reliable_updates)
+                    reliable_updates=self.reliable_updates, route=self.route)
 
 
 class StagError(RuntimeError):

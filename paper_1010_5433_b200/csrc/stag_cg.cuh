@@ -31,6 +31,7 @@ struct CgState {
     int done;               // 0 running | 1 finishing (x update of this iteration pending) | 2 over
     int converged, breakdown, stagnated, since_best;
     int zero_ok;            // N2 polish: stop >= 1 means "the zero start is good enough": 0 iterations
+    int replacements;       // N2 residual-replacement kernel: true-residual replacements done (read-back only)
     unsigned int ticket;    // last-block detection for the grid-wide reductions
 };
 

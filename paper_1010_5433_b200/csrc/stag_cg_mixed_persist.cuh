@@ -42,6 +42,7 @@ struct MixedExtra {            // scalars the mixed kernel needs on top of Scala
     double ca64[STAG_MAX_SHIFTS];   // alpha_i of the live shifts in fp64 (for the fp64 x_i)
     double a_base64, c0_64, rr_ru;
     int ru, verify, nru, last;
+    int stall;                      // consecutive replacements whose TRUE residual fell by less than 10 %
 };
 
 // SPLIT_HI: W_hi is a split-double buffer (N3) — typically the very buffer whose b planes are W_lo.
@@ -114,7 +115,7 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
             c.bb = bb; c.rr = bb; c.best_rr = bb; c.alpha = 0.0; c.alpha_old = 1.0; c.beta_old = 0.0;
             c.pq = 0.0; c.iter = 0; c.done = 0; c.converged = 0; c.breakdown = 0; c.stagnated = 0;
             c.since_best = 0; c.nlive = 0;
-            mx.c0_64 = st->c0; mx.rr_ru = bb; mx.ru = 0; mx.verify = 0; mx.nru = 0; mx.last = 0;
+            mx.c0_64 = st->c0; mx.rr_ru = bb; mx.ru = 0; mx.verify = 0; mx.nru = 0; mx.last = 0; mx.stall = 0;
             if (!(bb > 0.0)) { c.converged = (bb == 0.0); c.breakdown = !(bb == 0.0); c.done = 2; }
             else if (maxiter <= 0) c.done = 2;
         }
@@ -159,11 +160,18 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
             if (tid < 32) {
                 const double rr_true = grid_total(part_rr, G);
                 if (tid == 0) {
+                    // stagnation latch (reading A9 for this kernel): the recursive residual keeps falling and keeps
+                    // triggering replacements, but if the TRUE one has stopped following it — an unreachable stop, or
+                    // the fp32 rounding of the matrices — three replacements in a row that gain less than 10 % end
+                    // the run with stagnated = 1 and the polish takes over
+                    if (rr_true > 0.81 * mx.rr_ru) ++mx.stall; else mx.stall = 0;
                     c.rr = rr_true; mx.rr_ru = rr_true; mx.ru = 0; ++mx.nru;
+                    c.best_rr = rr_true; c.since_best = 0;
                     if (mx.verify) {
                         mx.verify = 0;
                         if (sqrt(rr_true / c.bb) <= c.stop) { c.converged = 1; c.done = 2; }
                     }
+                    if (c.done == 0 && mx.stall >= 3) { c.stagnated = 1; c.done = 2; }
                     if (mx.last || !(rr_true == rr_true)) { if (!(rr_true == rr_true)) c.breakdown = 1; c.done = 2; }
                 }
             }
@@ -283,6 +291,9 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
                 if (!(rr_new == rr_new)) { c.breakdown = 1; mx.ru = 1; mx.last = 1; }
                 else if (rel <= c.stop) { mx.ru = 1; mx.verify = 1; }              // convergence only on the TRUE residual
                 else if (rr_new < a.ru_delta * a.ru_delta * mx.rr_ru) mx.ru = 1;
+                else if (rr_new < c.best_rr) { c.best_rr = rr_new; c.since_best = 0; }
+                else if (++c.since_best >= 50) { mx.ru = 1; c.since_best = 0; }   // reading A9: the recursive residual has
+                                                                                 // stopped falling too — look at the true one
                 if (iter >= maxiter) { mx.ru = 1; mx.verify = 1; mx.last = 1; }
             }
         }
@@ -351,7 +362,7 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
         if (i == 0) {
             o->bb = c.bb; o->rr = c.rr; o->pq = c.pq; o->alpha = c.alpha;
             o->iter = c.iter; o->converged = c.converged; o->breakdown = c.breakdown;
-            o->stagnated = 0; o->since_best = mx.nru; o->done = 2;      // since_best carries the replacement count
+            o->stagnated = c.stagnated; o->replacements = mx.nru; o->done = 2;
         }
     }
 }

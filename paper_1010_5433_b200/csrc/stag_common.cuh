@@ -65,6 +65,7 @@ struct Options {
     int cg_resident_slices;  // persistent kernel: at most this many of r, q, p_base resident in shared memory (0..3)
     int cg_mixed_reliable;   // stag_mshift_cg_mixed: inner stage = persistent kernel with residual replacement: 0 never | 1 single shift | 2 always
     int cg_mixed_delta_inv;  // ... which replaces the residual whenever ||r|| has fallen by this factor (default 10)
+    int cg_mixed_fp64_from;  // stag_mshift_cg_mixed: from this many shifts on (and stop < 1e-6) the call is the fp64 multi-shift solve; 0 never
     int cg_persistent;       // 1: whole solve as one cooperative kernel when r,q,p fit in shared memory; 0: never
     int cg_l2_keep_mb;       // persistent kernel: MB of x_i, p_i (lightest shifts first) kept L2-resident (evict_last); 0: none
     int cg_fill;             // persistent kernel: 1 = deferred shift updates are worked off while waiting at sync points

@@ -41,6 +41,7 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
     c->opt.cg_resident_slices = 3;
     c->opt.cg_mixed_reliable = 1;
     c->opt.cg_mixed_delta_inv = 10;
+    c->opt.cg_mixed_fp64_from = 3;
     c->opt.cg_l2_keep_mb = 64;
     c->opt.cg_fill = 1;
     c->opt.cg_nbflags = 1;
@@ -91,6 +92,7 @@ static int *option_slot(Options &o, const char *key) {
     if (!std::strcmp(key, "cg_resident_slices")) return &o.cg_resident_slices;
     if (!std::strcmp(key, "cg_mixed_reliable")) return &o.cg_mixed_reliable;
     if (!std::strcmp(key, "cg_mixed_delta_inv")) return &o.cg_mixed_delta_inv;
+    if (!std::strcmp(key, "cg_mixed_fp64_from")) return &o.cg_mixed_fp64_from;
     if (!std::strcmp(key, "cg_l2_keep_mb")) return &o.cg_l2_keep_mb;
     if (!std::strcmp(key, "cg_fill")) return &o.cg_fill;
     if (!std::strcmp(key, "cg_nbflags")) return &o.cg_nbflags;
@@ -109,6 +111,7 @@ extern "C" int stag_set_option(stag_ctx *ctx, const char *key, int value) {
     if (slot == &ctx->opt.cg_check_every && value < 1) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_persistent_threads && value != 0 && value != 256 && value != 512 && value != 1024) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_mixed_delta_inv && value < 2) return STAG_ERR_BADARG;
+    if (slot == &ctx->opt.cg_mixed_fp64_from && (value < 0 || value > STAG_MAX_SHIFTS + 1)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_mixed_reliable && (value < 0 || value > 2)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_resident_slices && (value < 0 || value > 3)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_ctas_per_sm && (value < 1 || value > 16)) return STAG_ERR_BADARG;

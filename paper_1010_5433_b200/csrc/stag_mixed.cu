@@ -219,7 +219,7 @@ partial_fraction64_kernel(const long nchunk, const double2 *__restrict__ b, cons
     }
 }
 
-struct MixedLayout { size_t res, b32, x32, cg32, w64, polish, total; };
+struct MixedLayout { size_t res, b32, x32, cg32, w64, polish, total; };   // cg32 also holds the fp64 CG workspace of route 3
 
 static MixedLayout mixed_layout(const stag_ctx *ctx, int nshift) {
     MixedLayout l;
@@ -228,7 +228,7 @@ static MixedLayout mixed_layout(const stag_ctx *ctx, int nshift) {
     l.res = off;    off += 256;                                   // residues on the device
     l.b32 = off;    off += align256(v32);
     l.x32 = off;    off += align256(v32 * (size_t)nshift);
-    l.cg32 = off;   off += align256(cg_workspace_layout(ctx, STAG_F32, nshift, nullptr));
+    l.cg32 = off;   off += align256(cg_workspace_layout(ctx, STAG_F64, nshift, nullptr));   // >= the fp32 layout
     l.w64 = off;    off += align256((size_t)ctx->g.Vh * vec_bytes_per_site(STAG_F64));
     l.polish = off; off += polish_layout(ctx).total;
     l.total = off;
@@ -285,12 +285,13 @@ static int mixed_persistent(const stag_ctx *ctx, const void *packed_hi, int prec
     STAG_CUDA_OK(cudaStreamSynchronize(st));
     std::memset(info, 0, sizeof(*info));
     info->iters = h->iter; info->converged = h->converged; info->breakdown = h->breakdown;
+    info->stagnated = h->stagnated;
     info->bnorm2 = h->bb; info->rnorm2 = h->rr; info->kernel_launches = 1;
     for (int i = 0; i < nshift; ++i) {
         info->resid_iter[i] = h->bb > 0.0 ? h->resid_shift[i] : 0.0;
         info->iters_shift[i] = h->iters_shift[i];
     }
-    *replacements = h->since_best;
+    *replacements = h->replacements;
     if (h->breakdown) return STAG_ERR_BREAKDOWN;
     return h->converged ? STAG_OK : STAG_ERR_NOTCONV;
 }
@@ -369,6 +370,22 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     stag_mixed_info mi;
     std::memset(&mi, 0, sizeof(mi));
 
+    // Route (option "cg_mixed_fp64_from", default 3).  Measured at 32^3 x 8, stop 1e-10: one shift —
+    // residual replacement wins (0.105 against 0.17 s); two — fp32 + polish (0.163 against 0.178 s); from three or
+    // four shifts on the polish, which gives up the shared Krylov space (sum_i instead of max_i iterations), costs
+    // more than fp32 saved: the fp64 multi-shift solve is the fastest way to the fp64 stop, which is the paper's own
+    // conclusion for the Metropolis solves.  So from that many shifts on the call IS the fp64
+    // multi-shift solve on packed_hi, followed by the same true-residual check (and, if ever needed, polish).
+    const int fp64_from = ctx->opt.cg_mixed_fp64_from;
+    if (fp64_from > 0 && nshift >= fp64_from && stop < 1e-6) {
+        mi.route = 3;
+        const int crc = stag_mshift_cg(ctx, packed_hi, prec_hi, recon_hi, b_even, mass, nshift, host_shifts, nullptr, 0.0,
+                                       stop, maxiter, x_even, nullptr, ws + lay.cg32, &mi.inner, st);
+        if (crc != STAG_OK && crc != STAG_ERR_NOTCONV) {
+            if (info) *info = mi;
+            return crc;
+        }
+    } else {
     // inner stage, preferred form: one persistent kernel with residual replacement (fp32 matrices, fp64 x_i)
     int rc = STAG_ERR_UNSUPPORTED;
     // cg_mixed_reliable: 0 never | 1 (default) when it pays — a single shift, where nothing is left to polish
@@ -379,11 +396,13 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
         rc = mixed_persistent(ctx, packed_hi, prec_hi, packed_lo, recon_lo, b_even, mass, nshift, host_shifts, stop, maxiter,
                               x_even, ws, lay, &mi.inner, &mi.reliable_updates, st);
     if (rc != STAG_ERR_UNSUPPORTED) {
+        mi.route = 1;
         if (rc != STAG_OK && rc != STAG_ERR_NOTCONV) {
             if (info) *info = mi;
             return rc;
         }
     } else {
+    mi.route = 2;
     // plain fp32 stage: b -> fp32, multi-shift CG from zero, x -> fp64
     rc = stag_vector_convert(ctx, b_even, STAG_F64, ws + lay.b32, STAG_F32, 1, st);
     if (rc) return rc;
@@ -395,6 +414,7 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     }
     rc = stag_vector_convert(ctx, ws + lay.x32, STAG_F32, x_even, STAG_F64, nshift, st);
     if (rc) return rc;
+    }
     }
 
     // fp64 stage: per-shift defect-correction polish

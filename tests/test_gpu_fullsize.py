@@ -100,13 +100,14 @@ def test_c4_mixed_precision_on_one_split_buffer(stag, c4):
     cfg, U, srcs = c4
     L, m, shifts, stop = cfg["L"], cfg["mass"], cfg["shifts"], cfg["stops"][0]
     ctx = stag.Stag(L)
+    ctx.set_option("cg_mixed_fp64_from", 0)      # the fp32 + polish route (16 shifts would default to the fp64 solve)
     split = ctx.upload_gauge(U, stag.F64_SPLIT, 18)
     n, vb = len(shifts), ctx.vector_bytes(stag.F64)
     x, ws = ctx.alloc(n * vb), ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(n))
     b = srcs[2]
     rc, info = ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, ctx.upload_vector(b, stag.F64), m, shifts,
                                    stop, 100000, x, ws)
-    assert rc == 0, info
+    assert rc == 0 and info["route"] == 2, info
     nb = np.linalg.norm(b)
     for i, s in enumerate(shifts):
         xi = ctx.download_vector(x, stag.F64, i * vb)

@@ -97,6 +97,7 @@ def test_mixed_config1(stag, hi, recon_hi, recon_lo, reliable):
     L, U, b, m, shifts = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"], cfg["shifts"]
     ctx = stag.Stag(L)
     ctx.set_option("cg_mixed_reliable", reliable)
+    ctx.set_option("cg_mixed_fp64_from", 0)          # the fp32 routes are what is tested here (default: 4 shifts -> fp64)
     replaced = reliable == 2 and recon_hi == recon_lo
     prec_hi = getattr(stag, hi)
     p_hi = ctx.upload_gauge(U, prec_hi, recon_hi)
@@ -207,6 +208,60 @@ def test_mixed_config3_metropolis_stop_1e12(stag):
                 assert pinfo["iters"][i] == 0
     finally:
         oracle.set_threads(1)
+
+
+@pytest.mark.parametrize("hi", ["F64", "F64_SPLIT"])
+def test_mixed_default_route_is_the_fastest_one(stag, hi):
+    """Default options: 1 shift -> route 1 (residual replacement), 2 shifts -> route 2 (fp32 + polish), from 3 shifts
+    on -> route 3, the fp64 multi-shift solve itself (the paper's choice for the Metropolis solves):
+    then the iteration count is the oracle's +-2 and the polish finds nothing to do.  With a stop fp32 can reach the
+    fp32 routes are kept.  Every x_i must meet the stop by the oracle's operator on every route."""
+    cfg = si.get_config("c1_4x4x4x4")
+    L, U, b, m = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"]
+    all_shifts = [0.01, 0.04, 0.16, 0.64, 1.5]
+    ctx = stag.Stag(L)
+    prec_hi = getattr(stag, hi)
+    p_hi = ctx.upload_gauge(U, prec_hi, 18)
+    p_lo = p_hi if hi == "F64_SPLIT" else ctx.upload_gauge(U, stag.F32, 18)
+    vb = ctx.vector_bytes(stag.F64)
+    bdev = ctx.upload_vector(b, stag.F64)
+    for n, want in ((1, 1), (2, 2), (3, 3), (5, 3)):
+        shifts = all_shifts[:n]
+        x, ws = ctx.alloc(n * vb), ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(n))
+        rc, info = ctx.mshift_cg_mixed(p_hi, prec_hi, 18, p_lo, 18, bdev, m, shifts, 1e-10, 2000, x, ws)
+        assert rc == 0 and info["route"] == want, (n, info["route"])
+        for i, s in enumerate(shifts):
+            assert true_res(L, U, m, s, b, ctx.download_vector(x, stag.F64, i * vb)) <= 1e-10
+        if want == 3:
+            ref = oracle.mshift_cg(L, U, b, m, shifts, 1e-10, 2000)
+            assert abs(info["inner"]["iters"] - ref["iters"]) <= 2 and info["reliable_updates"] == 0
+            assert sum(info["polish"]["iters"]) == 0 and max(info["polish"]["resid_before"]) <= 1e-10
+    # a stop fp32 reaches: stays on the fp32 routes whatever the number of shifts
+    x, ws = ctx.alloc(5 * vb), ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(5))
+    rc, info = ctx.mshift_cg_mixed(p_hi, prec_hi, 18, p_lo, 18, bdev, m, all_shifts, 1e-5, 2000, x, ws)
+    assert rc == 0 and info["route"] == 2
+    ctx.set_option("cg_mixed_fp64_from", 0)
+    rc, info = ctx.mshift_cg_mixed(p_hi, prec_hi, 18, p_lo, 18, bdev, m, all_shifts, 1e-10, 2000, x, ws)
+    assert rc == 0 and info["route"] == 2 and max(info["polish"]["iters"]) > 0
+
+
+def test_mixed_residual_replacement_stagnation_latch(stag):
+    """A stop the true residual cannot reach (1e-18): the residual-replacement kernel must not run to maxiter — three
+    replacements in a row that gain less than 10 % latch stagnated = 1 — and the call reports NOTCONV with the
+    true residuals it reached (far below fp32's floor, since x and the replacements are fp64)."""
+    cfg = si.get_config("c1_4x4x4x4")
+    L, U, b, m = cfg["L"], si.make_links(cfg), si.make_source(cfg), cfg["mass"]
+    ctx = stag.Stag(L)
+    split = ctx.upload_gauge(U, stag.F64_SPLIT, 18)
+    vb = ctx.vector_bytes(stag.F64)
+    x, ws = ctx.alloc(vb), ctx.alloc(ctx.mshift_cg_mixed_workspace_bytes(1))
+    rc, info = ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, ctx.upload_vector(b, stag.F64), m, [0.01],
+                                   1e-18, 20000, x, ws)
+    assert rc == stag.ERR_NOTCONV and info["route"] == 1
+    assert info["inner"]["stagnated"] and not info["inner"]["converged"] and not info["inner"]["breakdown"]
+    assert info["inner"]["iters"] < 2000 and info["reliable_updates"] >= 3
+    assert info["polish"]["resid_after"][0] < 1e-12
+    assert true_res(L, U, m, 0.01, b, ctx.download_vector(x, stag.F64)) < 1e-12
 
 
 def test_mixed_bad_arguments(stag):
