@@ -32,8 +32,13 @@
  *              no exceptions, no exit().  Kernel launches are asynchronous: a launch error
  *              shows up as STAG_ERR_CUDA from the same or a later call.
  *   Aliasing   input and output buffers of one call must not overlap.
- *   Threads    a stag_ctx may be shared by calls on different streams, except that only one
- *              stag_mshift_cg* call may be in flight per ctx at a time.
+ *   Threads    a stag_ctx may be shared by host threads and by calls on different streams.  Every
+ *              synchronising call (stag_mshift_cg*, stag_cg_polish, recon-12 stag_gauge_pack, the
+ *              *_host calls) leases one of 4 host staging slots of the context for its duration, so
+ *              up to 4 of them run concurrently — the paper's independent pseudo-fermion solves
+ *               on separate streams — and a fifth waits for a free slot.  Calls that
+ *              run concurrently must not share output buffers or workspaces.  stag_set_option is
+ *              not synchronised with running calls.
  *
  * CANONICAL (interchange) FORMATS — always fp64
  *   site index   lex(x) = x0 + L0*(x1 + L1*(x2 + L2*x3));  one-parity index e = lex(x)/2

@@ -8,6 +8,8 @@
 //   a6  x_i += alpha_i p_i ; p_i = zeta_i r + beta_i p_i  for every active shift, one pass
 //                                                    cg_update_shifts_kernel
 // Vectors are T (fp64 or fp32); every reduction and scalar is fp64.
+#include <cstring>
+
 #include "stag_cg.cuh"
 
 namespace stag {
@@ -211,7 +213,7 @@ struct CgLaunch {
 // multi-kernel path: four launches per iteration, batches replayed as a CUDA graph, the host
 // polls the device-latched `done` word once per batch.
 template <typename T>
-static int run_multikernel(const CgLaunch<T> &L, const void *b, void *y, int maxiter, int *launches_out) {
+static int run_multikernel(const CgLaunch<T> &L, Slot &slot, const void *b, void *y, int maxiter, int *launches_out) {
     typedef CgLaunch<T> Lz;
     const stag_ctx *ctx = L.ctx;
     cudaStream_t st = L.st;
@@ -237,25 +239,38 @@ static int run_multikernel(const CgLaunch<T> &L, const void *b, void *y, int max
         if (rc) { cudaGetLastError(); return rc; }
     }
     if (ctx->opt.cg_graph && maxiter > 0 && !profile) {
-        cudaGraph_t graph = nullptr;
-        cudaStream_t cap = nullptr;
-        // capture on a private stream so the caller's stream (possibly the legacy default) is untouched
-        if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) return STAG_ERR_CUDA;
-        Lz Lc = L;
-        Lc.st = cap;
-        if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) rc = STAG_ERR_CUDA;
-        for (int j = 0; j < batch && rc == STAG_OK; ++j) rc = Lc.iteration();
-        if (cudaStreamEndCapture(cap, &graph) != cudaSuccess) rc = rc ? rc : STAG_ERR_CUDA;
-        if (rc == STAG_OK && cudaGraphInstantiate(&gexec, graph, 0) != cudaSuccess) rc = STAG_ERR_CUDA;
-        if (graph) cudaGraphDestroy(graph);
-        cudaStreamDestroy(cap);
-        if (rc) { cudaGetLastError(); return rc; }
+        // the instantiated graph of one batch is kept in the staging slot and replayed by every later solve whose
+        // launches would be identical (same buffers, storage and options: an MD trajectory makes hundreds of those)
+        GraphKey key;
+        std::memset(&key, 0, sizeof(key));
+        key.packed = L.packed; key.ws = L.ws; key.x = L.x;
+        key.prec = L.prec; key.recon = L.recon; key.nshift = L.nshift; key.base = L.base; key.batch = batch;
+        key.dslash_block = ctx->opt.dslash_block; key.dslash_regs = ctx->opt.dslash_regs;
+        key.dslash_ctas_per_sm = ctx->opt.dslash_ctas_per_sm; key.cg_ctas_per_sm = ctx->opt.cg_ctas_per_sm;
+        if (slot.gexec && std::memcmp(&key, &slot.key, sizeof(key)) != 0) {
+            cudaGraphExecDestroy(slot.gexec);
+            slot.gexec = nullptr;
+        }
+        if (!slot.gexec) {
+            cudaGraph_t graph = nullptr;
+            cudaStream_t cap = nullptr;
+            // capture on a private stream so the caller's stream (possibly the legacy default) is untouched
+            if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) return STAG_ERR_CUDA;
+            Lz Lc = L;
+            Lc.st = cap;
+            if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) rc = STAG_ERR_CUDA;
+            for (int j = 0; j < batch && rc == STAG_OK; ++j) rc = Lc.iteration();
+            if (cudaStreamEndCapture(cap, &graph) != cudaSuccess) rc = rc ? rc : STAG_ERR_CUDA;
+            if (rc == STAG_OK && cudaGraphInstantiate(&slot.gexec, graph, 0) != cudaSuccess) rc = STAG_ERR_CUDA;
+            if (graph) cudaGraphDestroy(graph);
+            cudaStreamDestroy(cap);
+            if (rc) { cudaGetLastError(); slot.gexec = nullptr; return rc; }
+            slot.key = key;
+        }
+        gexec = slot.gexec;
     }
-    volatile int *poll = ctx->pinned_flags + 8;      // two slots: poll[0], poll[1]
-    cudaEvent_t ev[2] = {nullptr, nullptr};
-    if (cudaEventCreateWithFlags(&ev[0], cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&ev[1], cudaEventDisableTiming) != cudaSuccess)
-        rc = STAG_ERR_CUDA;
+    volatile int *poll = slot.pinned_flags + 8;      // two words: poll[0], poll[1]
+    cudaEvent_t *ev = slot.ev;
     const int nbatch = (maxiter + batch - 1) / batch;
     int launches = 1;
     for (int k = 0; k <= nbatch && rc == STAG_OK; ++k) {
@@ -282,9 +297,6 @@ static int run_multikernel(const CgLaunch<T> &L, const void *b, void *y, int max
             else if (poll[(k - 1) & 1] != 0) break;
         }
     }
-    if (ev[0]) cudaEventDestroy(ev[0]);
-    if (ev[1]) cudaEventDestroy(ev[1]);
-    if (gexec) cudaGraphExecDestroy(gexec);
     if (profile) {
         double sum[4] = {0.0, 0.0, 0.0, 0.0};
         if (rc == STAG_OK && nprof > 0 && cudaEventSynchronize(pev[nprof - 1][4]) == cudaSuccess) {
@@ -313,7 +325,7 @@ static int run_multikernel(const CgLaunch<T> &L, const void *b, void *y, int max
 }
 
 template <typename T>
-static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, const void *b,
+static int run_cg(const stag_ctx *ctx, Slot &slot, const void *packed, int prec, int recon, const void *b,
                   double mass, int nshift, const double *shifts, const double *residues,
                   double residue0, double stop, int maxiter, void *x, void *y, void *workspace,
                   stag_cg_info *info, cudaStream_t st) {
@@ -339,7 +351,7 @@ static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, 
     L.base = base;
 
     // initial state, staged through the ctx's pinned buffer
-    CgState *h = static_cast<CgState *>(ctx->pinned_info);
+    CgState *h = static_cast<CgState *>(slot.pinned_info);
     memset(h, 0, sizeof(*h));
     h->alpha_old = 1.0; h->beta_old = 0.0;
     h->c0 = mass * mass + shifts[base];
@@ -365,7 +377,7 @@ static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, 
         else launches = 1;
     }
     if (!persistent) {
-        const int mrc = run_multikernel(L, b, y, maxiter, &launches);
+        const int mrc = run_multikernel(L, slot, b, y, maxiter, &launches);
         if (mrc) return mrc;
     }
     STAG_CUDA_OK(cudaMemcpyAsync(h, L.state, sizeof(CgState), cudaMemcpyDeviceToHost, st));
@@ -393,11 +405,11 @@ static int run_cg(const stag_ctx *ctx, const void *packed, int prec, int recon, 
 
 using namespace stag;
 
-extern "C" int stag_mshift_cg(const stag_ctx *ctx, const void *packed, int prec, int recon,
-                              const void *b_even, double mass, int nshift,
-                              const double *host_shifts, const double *host_residues,
-                              double residue0, double stop, int maxiter, void *x_even,
-                              void *y_even, void *workspace, stag_cg_info *info, void *stream) {
+int stag::mshift_cg_impl(const stag_ctx *ctx, Slot &slot, const void *packed, int prec, int recon,
+                         const void *b_even, double mass, int nshift,
+                         const double *host_shifts, const double *host_residues,
+                         double residue0, double stop, int maxiter, void *x_even,
+                         void *y_even, void *workspace, stag_cg_info *info, void *stream) {
     if (!ctx || !packed || !b_even || !host_shifts || !x_even || !workspace) return STAG_ERR_BADARG;
     if (!valid_prec(prec) || !valid_recon(recon)) return STAG_ERR_BADARG;
     if (nshift < 1 || nshift > STAG_MAX_SHIFTS || !(stop > 0.0) || maxiter < 0) return STAG_ERR_BADARG;
@@ -411,9 +423,20 @@ extern "C" int stag_mshift_cg(const stag_ctx *ctx, const void *packed, int prec,
     if (((uintptr_t)workspace & 255) != 0) return STAG_ERR_BADARG;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     if (prec != STAG_F32)
-        return run_cg<double>(ctx, packed, prec, recon, b_even, mass, nshift, host_shifts,
+        return run_cg<double>(ctx, slot, packed, prec, recon, b_even, mass, nshift, host_shifts,
                               host_residues, residue0, stop, maxiter, x_even, y_even, workspace,
                               info, st);
-    return run_cg<float>(ctx, packed, prec, recon, b_even, mass, nshift, host_shifts, host_residues,
+    return run_cg<float>(ctx, slot, packed, prec, recon, b_even, mass, nshift, host_shifts, host_residues,
                          residue0, stop, maxiter, x_even, y_even, workspace, info, st);
+}
+
+extern "C" int stag_mshift_cg(const stag_ctx *ctx, const void *packed, int prec, int recon,
+                              const void *b_even, double mass, int nshift,
+                              const double *host_shifts, const double *host_residues,
+                              double residue0, double stop, int maxiter, void *x_even,
+                              void *y_even, void *workspace, stag_cg_info *info, void *stream) {
+    if (!ctx) return STAG_ERR_BADARG;
+    SlotLease lease(ctx);
+    return mshift_cg_impl(ctx, lease.slot(), packed, prec, recon, b_even, mass, nshift, host_shifts, host_residues,
+                          residue0, stop, maxiter, x_even, y_even, workspace, info, stream);
 }

@@ -141,11 +141,17 @@ int dslash_oe_cg_dispatch(const stag_ctx *ctx, const void *packed, int prec, int
 // implemented in stag_cg_persist.cu: nrhs independent sources in one persistent launch.  src_sigma /
 // src_stop (nullable): N2 polish — nshift must be 1 and source s solves (A + src_sigma[s]) e = b_s to
 // src_stop[s]; a source whose src_stop[s] >= 1 returns e = 0 after 0 iterations.
-int block_solve(const stag_ctx *ctx, const void *packed, int prec, int recon, int nrhs, const void *b_even,
+int block_solve(const stag_ctx *ctx, Slot &slot, const void *packed, int prec, int recon, int nrhs, const void *b_even,
                 double mass, int nshift, const double *host_shifts, const double *src_sigma,
                 const double *src_stop, const double *host_residues, double residue0, double stop,
                 int maxiter, void *x_even, void *y_even, void *workspace, stag_cg_info *info,
                 cudaStream_t st);
+
+// stag_mshift_cg on a staging slot the caller has leased (stag_cg.cu)
+int mshift_cg_impl(const stag_ctx *ctx, Slot &slot, const void *packed, int prec, int recon, const void *b_even,
+                   double mass, int nshift, const double *host_shifts, const double *host_residues, double residue0,
+                   double stop, int maxiter, void *x_even, void *y_even, void *workspace, stag_cg_info *info,
+                   void *stream);
 
 // implemented in stag_cg_persist.cu: the whole solve as one cooperative kernel (small lattices)
 bool cg_persistent_fits(const stag_ctx *ctx, int prec);

@@ -96,12 +96,13 @@ extern "C" int stag_mshift_cg_block(const stag_ctx *ctx, const void *packed, int
     }
     if (!(mass * mass + smin > 0.0)) return STAG_ERR_BADARG;
     if (((uintptr_t)workspace & 255) != 0) return STAG_ERR_BADARG;
-    return block_solve(ctx, packed, prec, recon, nrhs, b_even, mass, nshift, host_shifts, nullptr, nullptr,
+    SlotLease lease(ctx);
+    return block_solve(ctx, lease.slot(), packed, prec, recon, nrhs, b_even, mass, nshift, host_shifts, nullptr, nullptr,
                        host_residues, residue0, stop, maxiter, x_even, y_even, workspace, info,
                        static_cast<cudaStream_t>(stream));
 }
 
-int stag::block_solve(const stag_ctx *ctx, const void *packed, int prec, int recon, int nrhs, const void *b_even,
+int stag::block_solve(const stag_ctx *ctx, Slot &slot, const void *packed, int prec, int recon, int nrhs, const void *b_even,
                       double mass, int nshift, const double *host_shifts, const double *src_sigma,
                       const double *src_stop, const double *host_residues, double residue0, double stop,
                       int maxiter, void *x_even, void *y_even, void *workspace, stag_cg_info *info,
@@ -114,7 +115,7 @@ int stag::block_solve(const stag_ctx *ctx, const void *packed, int prec, int rec
     const size_t vbytes = (size_t)ctx->g.Vh * vec_bytes_per_site(prec);
 
     // initial state: the same for every source, staged through the ctx's pinned buffer
-    CgState *h = static_cast<CgState *>(ctx->pinned_info);
+    CgState *h = static_cast<CgState *>(slot.pinned_info);
     std::memset(h, 0, sizeof(*h));
     h->alpha_old = 1.0;
     h->c0 = mass * mass + host_shifts[base];

@@ -5,6 +5,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <condition_variable>
+#include <mutex>
+
 #include "../../include/stag.h"
 
 namespace stag {
@@ -75,13 +78,35 @@ struct Options {
 
 }  // namespace stag
 
+namespace stag {
+// Host-side staging of ONE synchronising call (stag_mshift_cg*, stag_cg_polish, recon-12 stag_gauge_pack): pinned
+// memory for the state upload / read-back and the convergence polls, and the cached CUDA graph of the multi-kernel
+// CG path.  A context owns a small pool of these; a call leases one for its whole duration, so independent
+// solves — the paper's several pseudo-fermions — may run concurrently on different streams of one
+// context, and back-to-back solves with the same buffers replay the graph instead of re-capturing it.
+struct GraphKey {                 // everything the captured launches depend on
+    const void *packed; void *ws; void *x;
+    int prec, recon, nshift, base, batch, dslash_block, dslash_regs, dslash_ctas_per_sm, cg_ctas_per_sm;
+};
+struct Slot {
+    int *pinned_flags;            // 512 B pinned (mapped): status words, convergence polls; bytes 128.. = 16 doubles (N2 norms)
+    void *pinned_info;            // pinned staging for the CG state upload / read-back (one CgState)
+    cudaGraphExec_t gexec;        // multi-kernel path: one batch of cg_check_every iterations, for `key`
+    GraphKey key;
+    cudaEvent_t ev[2];            // poll events of the multi-kernel path
+    bool busy;
+};
+static constexpr int kSlots = 4;
+}  // namespace stag
+
 struct stag_ctx {
     stag::Geom g;
     stag::Options opt;
     int device;
     int num_sms;
-    int *pinned_flags;   // 512 B pinned (mapped) host buffer: status words, convergence polls; bytes 128.. = 16 doubles (N2 norms)
-    void *pinned_info;   // pinned staging for the CG state upload / read-back (one CgState)
+    mutable stag::Slot slots[stag::kSlots];
+    mutable std::mutex mu;
+    mutable std::condition_variable cv;
     // measurement aids (stag_kernel_log, stag_cg_profile): which kernels the calls on this ctx launched, and the
     // per-kernel times of the last profiled multi-kernel solve
     mutable const void *klog[32];
@@ -98,8 +123,33 @@ namespace stag {
         if (e__ != cudaSuccess) return STAG_ERR_CUDA;       \
     } while (0)
 
+// lease of one staging slot for the duration of a synchronising call (waits if all kSlots are in use)
+class SlotLease {
+    const stag_ctx *ctx_;
+    Slot *s_;
+public:
+    explicit SlotLease(const stag_ctx *ctx) : ctx_(ctx), s_(nullptr) {
+        std::unique_lock<std::mutex> lk(ctx->mu);
+        for (;;) {
+            for (int i = 0; i < kSlots; ++i)
+                if (!ctx->slots[i].busy) { s_ = &ctx->slots[i]; break; }
+            if (s_) break;
+            ctx->cv.wait(lk);
+        }
+        s_->busy = true;
+    }
+    ~SlotLease() {
+        { std::lock_guard<std::mutex> lk(ctx_->mu); s_->busy = false; }
+        ctx_->cv.notify_one();
+    }
+    SlotLease(const SlotLease &) = delete;
+    SlotLease &operator=(const SlotLease &) = delete;
+    Slot &slot() const { return *s_; }
+};
+
 // remember that `func` (a __global__ function) was launched on behalf of ctx (stag_kernel_log)
 inline void log_kernel(const stag_ctx *ctx, const void *func) {
+    std::lock_guard<std::mutex> lk(ctx->mu);
     for (int i = 0; i < ctx->nklog; ++i)
         if (ctx->klog[i] == func) return;
     if (ctx->nklog < 32) ctx->klog[ctx->nklog++] = func;

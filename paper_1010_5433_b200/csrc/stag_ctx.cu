@@ -17,9 +17,12 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
         V *= L[mu];
         if (V >= (1ll << 31)) return STAG_ERR_UNSUPPORTED;
     }
-    stag_ctx *c = new (std::nothrow) stag_ctx;
+    stag_ctx *c = new (std::nothrow) stag_ctx();
     if (!c) return STAG_ERR_CUDA;
-    std::memset(c, 0, sizeof(*c));
+    std::memset(&c->g, 0, sizeof(c->g));
+    std::memset(&c->opt, 0, sizeof(c->opt));
+    std::memset(c->slots, 0, sizeof(c->slots));
+    c->nklog = 0; c->prof_iters = 0;
     Geom &g = c->g;
     for (int mu = 0; mu < 4; ++mu) g.L[mu] = L[mu];
     g.Lh0 = L[0] / 2;
@@ -45,10 +48,16 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
     c->opt.cg_l2_keep_mb = 64;
     c->opt.cg_fill = 1;
     c->opt.cg_nbflags = 1;
-    if (cudaGetDevice(&c->device) != cudaSuccess ||
-        cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess ||
-        cudaHostAlloc((void **)&c->pinned_flags, 512, cudaHostAllocMapped) != cudaSuccess ||
-        cudaHostAlloc(&c->pinned_info, sizeof(CgState), cudaHostAllocDefault) != cudaSuccess) {
+    bool ok = cudaGetDevice(&c->device) == cudaSuccess &&
+              cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess;
+    for (int i = 0; i < kSlots && ok; ++i) {
+        Slot &s = c->slots[i];
+        ok = cudaHostAlloc((void **)&s.pinned_flags, 512, cudaHostAllocMapped) == cudaSuccess &&
+             cudaHostAlloc(&s.pinned_info, sizeof(CgState), cudaHostAllocDefault) == cudaSuccess &&
+             cudaEventCreateWithFlags(&s.ev[0], cudaEventDisableTiming) == cudaSuccess &&
+             cudaEventCreateWithFlags(&s.ev[1], cudaEventDisableTiming) == cudaSuccess;
+    }
+    if (!ok) {
         cudaGetLastError();
         stag_ctx_destroy(c);
         return STAG_ERR_CUDA;
@@ -59,8 +68,14 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
 
 extern "C" void stag_ctx_destroy(stag_ctx *ctx) {
     if (!ctx) return;
-    if (ctx->pinned_flags) cudaFreeHost(ctx->pinned_flags);
-    if (ctx->pinned_info) cudaFreeHost(ctx->pinned_info);
+    for (int i = 0; i < kSlots; ++i) {
+        Slot &s = ctx->slots[i];
+        if (s.gexec) cudaGraphExecDestroy(s.gexec);
+        if (s.ev[0]) cudaEventDestroy(s.ev[0]);
+        if (s.ev[1]) cudaEventDestroy(s.ev[1]);
+        if (s.pinned_flags) cudaFreeHost(s.pinned_flags);
+        if (s.pinned_info) cudaFreeHost(s.pinned_info);
+    }
     delete ctx;
 }
 

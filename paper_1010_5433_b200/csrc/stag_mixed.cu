@@ -107,7 +107,7 @@ static int dslash_n(const stag_ctx *ctx, const void *packed, int prec, int recon
     return STAG_OK;
 }
 
-static int polish(const stag_ctx *ctx, const void *packed, int prec, int recon, const char *b, double mass,
+static int polish(const stag_ctx *ctx, Slot &slot, const void *packed, int prec, int recon, const char *b, double mass,
                   int nshift, const double *shifts, double stop, int maxiter, char *x, char *ws,
                   stag_polish_info *info, cudaStream_t st) {
     const PolishLayout lay = polish_layout(ctx);
@@ -118,7 +118,7 @@ static int polish(const stag_ctx *ctx, const void *packed, int prec, int recon, 
     double *scal = reinterpret_cast<double *>(ws + lay.scal);
     unsigned int *ticket = reinterpret_cast<unsigned int *>(ws + lay.scal + 128);
     double *partials = reinterpret_cast<double *>(ws + lay.partials);
-    volatile double *hn = reinterpret_cast<volatile double *>(reinterpret_cast<char *>(ctx->pinned_flags) + 128);
+    volatile double *hn = reinterpret_cast<volatile double *>(reinterpret_cast<char *>(slot.pinned_flags) + 128);
     const int group = STAG_MAX_RHS;    // the defects of a split-double group are one Dslash launch per shift (dslash_n)
     stag_polish_info pi;
     std::memset(&pi, 0, sizeof(pi));
@@ -175,7 +175,7 @@ static int polish(const stag_ctx *ctx, const void *packed, int prec, int recon, 
             if (!any) break;
             if (pi.passes < pass) pi.passes = pass;
             stag_cg_info ci[STAG_MAX_RHS];
-            rc = block_solve(ctx, packed, prec, recon, n, ws + lay.r, mass, 1, sigma, sigma, sstop, nullptr, 0.0,
+            rc = block_solve(ctx, slot, packed, prec, recon, n, ws + lay.r, mass, 1, sigma, sigma, sstop, nullptr, 0.0,
                              stop, maxiter, ws + lay.e, nullptr, ws + lay.cg, ci, st);
             ++launches;
             if (rc == STAG_ERR_BREAKDOWN) worst = rc;
@@ -238,7 +238,7 @@ static MixedLayout mixed_layout(const stag_ctx *ctx, int nshift) {
 // The inner stage as ONE persistent kernel with residual replacement (stag_cg_mixed_persist.cuh): fp32 matrices
 // and directions, fp64 solutions, true fp64 residual of the base system at every replacement.  Returns
 // STAG_ERR_UNSUPPORTED when that kernel does not apply (the caller then runs the plain fp32 stage).
-static int mixed_persistent(const stag_ctx *ctx, const void *packed_hi, int prec_hi, const void *packed_lo, int recon,
+static int mixed_persistent(const stag_ctx *ctx, Slot &slot, const void *packed_hi, int prec_hi, const void *packed_lo, int recon,
                             const void *b64, double mass, int nshift, const double *shifts, double stop,
                             int maxiter, void *x64, char *ws, const MixedLayout &lay, stag_cg_info *info,
                             int *replacements, cudaStream_t st) {
@@ -249,7 +249,7 @@ static int mixed_persistent(const stag_ctx *ctx, const void *packed_hi, int prec
     int base = 0;
     for (int i = 1; i < nshift; ++i)
         if (shifts[i] < shifts[base]) base = i;
-    CgState *h = static_cast<CgState *>(ctx->pinned_info);
+    CgState *h = static_cast<CgState *>(slot.pinned_info);
     std::memset(h, 0, sizeof(*h));
     h->alpha_old = 1.0;
     h->c0 = mass * mass + shifts[base];
@@ -342,7 +342,8 @@ extern "C" int stag_cg_polish(const stag_ctx *ctx, const void *packed, int prec,
     const int bad = check_solve_args(ctx, packed, recon, b_even, mass, nshift, host_shifts, stop, maxiter, x_even, workspace);
     if (bad) return bad;
     if (prec != STAG_F64 && prec != STAG_F64_SPLIT) return STAG_ERR_BADARG;
-    return polish(ctx, packed, prec, recon, static_cast<const char *>(b_even), mass, nshift, host_shifts, stop,
+    SlotLease lease(ctx);
+    return polish(ctx, lease.slot(), packed, prec, recon, static_cast<const char *>(b_even), mass, nshift, host_shifts, stop,
                   maxiter, static_cast<char *>(x_even), static_cast<char *>(workspace), info,
                   static_cast<cudaStream_t>(stream));
 }
@@ -369,6 +370,8 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     const MixedLayout lay = mixed_layout(ctx, nshift);
     stag_mixed_info mi;
     std::memset(&mi, 0, sizeof(mi));
+    SlotLease lease(ctx);
+    Slot &slot = lease.slot();
 
     // Route (option "cg_mixed_fp64_from", default 3).  Measured at 32^3 x 8, stop 1e-10: one shift —
     // residual replacement wins (0.105 against 0.17 s); two — fp32 + polish (0.163 against 0.178 s); from three or
@@ -379,7 +382,7 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     const int fp64_from = ctx->opt.cg_mixed_fp64_from;
     if (fp64_from > 0 && nshift >= fp64_from && stop < 1e-6) {
         mi.route = 3;
-        const int crc = stag_mshift_cg(ctx, packed_hi, prec_hi, recon_hi, b_even, mass, nshift, host_shifts, nullptr, 0.0,
+        const int crc = mshift_cg_impl(ctx, slot, packed_hi, prec_hi, recon_hi, b_even, mass, nshift, host_shifts, nullptr, 0.0,
                                        stop, maxiter, x_even, nullptr, ws + lay.cg32, &mi.inner, st);
         if (crc != STAG_OK && crc != STAG_ERR_NOTCONV) {
             if (info) *info = mi;
@@ -393,7 +396,7 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     // rounding of the matrices times ||x_i||/||b|| and the polish costs as much as after the plain fp32 run) | 2 always
     const bool want_ru = ctx->opt.cg_mixed_reliable == 2 || (ctx->opt.cg_mixed_reliable == 1 && nshift == 1);
     if (want_ru && ctx->opt.cg_persistent && recon_hi == recon_lo)
-        rc = mixed_persistent(ctx, packed_hi, prec_hi, packed_lo, recon_lo, b_even, mass, nshift, host_shifts, stop, maxiter,
+        rc = mixed_persistent(ctx, slot, packed_hi, prec_hi, packed_lo, recon_lo, b_even, mass, nshift, host_shifts, stop, maxiter,
                               x_even, ws, lay, &mi.inner, &mi.reliable_updates, st);
     if (rc != STAG_ERR_UNSUPPORTED) {
         mi.route = 1;
@@ -406,7 +409,7 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     // plain fp32 stage: b -> fp32, multi-shift CG from zero, x -> fp64
     rc = stag_vector_convert(ctx, b_even, STAG_F64, ws + lay.b32, STAG_F32, 1, st);
     if (rc) return rc;
-    rc = stag_mshift_cg(ctx, packed_lo, STAG_F32, recon_lo, ws + lay.b32, mass, nshift, host_shifts, nullptr, 0.0,
+    rc = mshift_cg_impl(ctx, slot, packed_lo, STAG_F32, recon_lo, ws + lay.b32, mass, nshift, host_shifts, nullptr, 0.0,
                         inner_stop, maxiter, ws + lay.x32, nullptr, ws + lay.cg32, &mi.inner, st);
     if (rc != STAG_OK && rc != STAG_ERR_NOTCONV) {            // breakdown or a real error: nothing to polish
         if (info) *info = mi;
@@ -418,7 +421,7 @@ extern "C" int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, 
     }
 
     // fp64 stage: per-shift defect-correction polish
-    const int prc = polish(ctx, packed_hi, prec_hi, recon_hi, static_cast<const char *>(b_even), mass, nshift,
+    const int prc = polish(ctx, slot, packed_hi, prec_hi, recon_hi, static_cast<const char *>(b_even), mass, nshift,
                            host_shifts, stop, maxiter, static_cast<char *>(x_even), ws + lay.polish, &mi.polish, st);
     if (prc != STAG_OK && prc != STAG_ERR_NOTCONV && prc != STAG_ERR_BREAKDOWN) return prc;
 

@@ -170,10 +170,12 @@ extern "C" int stag_gauge_pack(const stag_ctx *ctx, const double *dev_links_cano
     const dim3 grid((g.Vh + 127) / 128, 16), block(128);
     char *out = static_cast<char *>(dev_packed);
     int *flag = nullptr;
+    // recon 12: the SU(3) check writes a mapped pinned status word of a leased staging slot
+    SlotLease lease(ctx);
+    int *host_flag = lease.slot().pinned_flags;
     if (recon == 12) {
-        // SU(3) check flag: ctx's mapped pinned status word (one recon-12 pack per ctx at a time)
-        STAG_CUDA_OK(cudaHostGetDevicePointer((void **)&flag, ctx->pinned_flags, 0));
-        ctx->pinned_flags[0] = 0;
+        STAG_CUDA_OK(cudaHostGetDevicePointer((void **)&flag, host_flag, 0));
+        host_flag[0] = 0;
     }
     if (prec == STAG_F64_SPLIT) {
         if (recon == 18) gauge_pack_kernel<SplitTag, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
@@ -188,7 +190,7 @@ extern "C" int stag_gauge_pack(const stag_ctx *ctx, const double *dev_links_cano
     STAG_CUDA_OK(cudaGetLastError());
     if (recon == 12) {
         STAG_CUDA_OK(cudaStreamSynchronize(st));
-        if (ctx->pinned_flags[0] != 0) return STAG_ERR_NOT_SU3;
+        if (host_flag[0] != 0) return STAG_ERR_NOT_SU3;
     }
     return STAG_OK;
 }
