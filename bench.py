@@ -462,10 +462,11 @@ def measure_block(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak
 
 
 def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
-    """N2 + N3: stag_mshift_cg_mixed with DEFAULT options on ONE resident split-double buffer (fp32 reads its b planes,
-    fp64 reads b + c) against stag_mshift_cg in fp64 on native fp64 links, for the lightest 1, 2, 4, 8, 16 shifts of
-    the workload, same source and stop; the call picks its route (1 residual replacement | 2 fp32 + polish | 3 fp64
-    multi-shift).  Then the fp32 + polish route forced at all 16 shifts, for the record."""
+    """N2 + N3: stag_mshift_cg_mixed with DEFAULT options (fp64 stages on the native fp64 links, fp32 stages on the b
+    planes of a split-double buffer) against stag_mshift_cg in fp64 on the same fp64 links, for the lightest 1, 2, 4,
+    8, 16 shifts of the workload, same source and stop; the call picks its route (1 residual replacement | 2 fp32 +
+    polish | 3 the fp64 multi-shift solve itself, plus the true-residual check).  Then, for the record, everything on
+    ONE resident split-double buffer (N3: its fp64 stages read b + c), and the fp32 + polish route forced at all shifts."""
     n = len(cfg["shifts"])
     split = ctx.upload_gauge(U, stag.F64_SPLIT, 18)
     p64 = ctx.upload_gauge(U, stag.F64, 18)
@@ -478,12 +479,17 @@ def measure_mixed(torch, stag, ctx, cfg, U, srcs, vh, fp64_s_per_solve):
     for k in sorted({1, 2, 4, 8, n} & set(range(1, n + 1))):
         sh = cfg["shifts"][:k]
         t64, (rc64, i64) = timed_call(torch, lambda: ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], sh, cfg["stops"][0], 100000, x, cgws))
-        tm, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], sh,
+        tm, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(p64, stag.F64, 18, split, 18, b, cfg["mass"], sh,
                                                                        cfg["stops"][0], 100000, x, ws))
         out["by_nshift"][str(k)] = {
             "rc": rc, "route": info["route"], "s_per_solve": tm, "fp64_s_per_solve": t64, "vs_fp64_multishift": t64 / tm,
             "inner_iters": info["inner"]["iters"], "fp64_iters": i64["iters"], "reliable_updates": info["reliable_updates"],
             "polish_iters": sum(info["polish"]["iters"]), "true_resid_final": max(info["polish"]["resid_after"])}
+    secs, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], cfg["shifts"],
+                                                                     cfg["stops"][0], 100000, x, ws))
+    out["one_split_buffer_all_shifts"] = {"rc": rc, "route": info["route"], "s_per_solve": secs,
+                                          "vs_fp64_multishift_native_links": fp64_s_per_solve / secs,
+                                          "true_resid_final": max(info["polish"]["resid_after"])}
     ctx.set_option("cg_mixed_fp64_from", 0)
     secs, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg_mixed(split, stag.F64_SPLIT, 18, split, 18, b, cfg["mass"], cfg["shifts"],
                                                                      cfg["stops"][0], 100000, x, ws))
@@ -753,7 +759,7 @@ def run_ours(args):
                                        have={(prec, recon): packed})
         also += ents
         if roof is None:
-            roof = next(e for e in ents if e.get("workload") == wl and name in e["what"])
+            roof = dict(next(e for e in ents if e.get("workload") == wl and name in e["what"]))   # multi-kernel path: the Dslash
         # ---- the solve in the other storage variants (fp32 / 12-real need driver-visible figures) ----
         solves = {}
         if not args.no_block and prec == stag.F64 and recon == 18:
