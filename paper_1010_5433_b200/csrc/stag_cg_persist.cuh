@@ -612,20 +612,16 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             __syncthreads();
             if (swap_rq) { const Slice<T> t = r_s; r_s = q_s; q_s = t; }       // the new r is where q was
             if (act2) {   // base shift first: its new p is what phase A of the next iteration gathers
-                const T ab = sc[rhs].a_base, zb = sc[rhs].z_base, bb_ = sc[rhs].b_base;
-                const uint64_t pol_base = shift_policy(base);
+                // (x_base += alpha p_base was already done while waiting at the sync point before: the base shift has
+                // theta = 1, so its alpha_i is alpha itself and needs only the first reduction)
+                const T zb = sc[rhs].z_base, bb_ = sc[rhs].b_base;
                 for (int ls = l0; ls < ns; ls += LS) {
                     const int e = e0 + ls, slot = rhs * S + ls;
-                    T rv[6], pv[6], xv[6];
-                    load_vec_pol(x_base, Vh, e, xv, pol_base);
+                    T rv[6], pv[6];
                     r_s.load(slot, rhs, Vh, e, rv);
                     p_s.load(slot, rhs, Vh, e, pv);
 #pragma unroll
-                    for (int k = 0; k < 6; ++k) {
-                        xv[k] = fma(ab, pv[k], xv[k]);
-                        pv[k] = fma(zb, rv[k], bb_ * pv[k]);
-                    }
-                    store_vec_pol(x_base, Vh, e, xv, pol_base);
+                    for (int k = 0; k < 6; ++k) pv[k] = fma(zb, rv[k], bb_ * pv[k]);
                     if (p_s.res) p_s.s.store(slot, pv);
                     store_vec(p_base, Vh, e, pv);
                 }
@@ -656,6 +652,8 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
         // acquire on to them.
         // Pending items MUST be finished (force) before phase D rewrites their coefficients, before phase C when
         // it overwrites the r they read (no swap), at the end of the solve — and at once if filling is off.
+        // Arrivals are release operations (red.release / st.release: MEMBAR.ALL, no L1 invalidation) instead of
+        // __threadfence() + a relaxed one (MEMBAR.SC + CCTL.IVALL).
         {
             const bool global = phase == 1 || phase == 2;
             __syncthreads();                               // this phase's writes are issued; n_running is visible
@@ -664,17 +662,18 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
             unsigned int target;
             if (global) {
                 target = ++gepoch * (unsigned)G;
-                if (tid == 0) { __threadfence(); atomicAdd(bar, 1u); }
+                if (tid == 0) asm volatile("red.release.gpu.global.add.u32 [%0], %1;" :: "l"(bar), "r"(1u) : "memory");
             } else {
                 target = ++nepoch;
                 if (tid == 0) {
-                    __threadfence();
-                    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" :: "l"(a.flags + (size_t)blockIdx.x * 32), "r"(target) : "memory");
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(a.flags + (size_t)blockIdx.x * 32), "r"(target) : "memory");
                 }
             }
             const bool poll_warp = tid < 32;
             bool released = false;
-            while (!released || (force && ppass < pnpass)) {
+            const int xbn = (phase == 2 && act2) ? (ns + LS - 1) / LS : 0;
+            int xbpass = 0;
+            while (!released || (force && ppass < pnpass) || xbpass < xbn) {
                 unsigned int v = target;
                 if (poll_warp && !released) {
                     if (global) {
@@ -721,6 +720,22 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                     pj += B;
                     if (pj >= pn) { pj = 0; ++ppass; }
                 }
+                else if (xbpass < xbn) {                   // x_base += alpha p_base: needs alpha only (theta_base = 1), so it
+                                                           // runs here, in the wait for <r,r>, instead of in phase D
+                    const int ls = l0 + xbpass * LS;
+                    if (ls < ns) {
+                        const int e = e0 + ls, slot = rhs * S + ls;
+                        const uint64_t pol = shift_policy(base);
+                        const T ab = (T)sc[rhs].alpha;
+                        T pv[6], xv[6];
+                        load_vec_pol(x_base, Vh, e, xv, pol);
+                        p_s.load(slot, rhs, Vh, e, pv);
+#pragma unroll
+                        for (int k = 0; k < 6; ++k) xv[k] = fma(ab, pv[k], xv[k]);
+                        store_vec_pol(x_base, Vh, e, xv, pol);
+                    }
+                    ++xbpass;
+                }
                 if (poll_warp) {
                     if (!released && __all_sync(0xffffffffu, (int)(v - target) >= 0)) {
                         if (tid == 0) {
@@ -732,7 +747,7 @@ cg_persistent_kernel(const Geom g, const PersistArgs a) {
                 } else {
                     // the other warps: released once warp 0 has seen the arrivals, or when out of items (the
                     // closing CTA barrier then waits in hardware instead of spinning)
-                    released = ppass >= pnpass || *reinterpret_cast<volatile unsigned int *>(&sync_seen) == sync_id;
+                    released = (ppass >= pnpass && xbpass >= xbn) || *reinterpret_cast<volatile unsigned int *>(&sync_seen) == sync_id;
                 }
             }
             __syncthreads();
