@@ -655,21 +655,26 @@ def ncu_pass(args, torch, stag, ctx, cfg, U, srcs, vh):
              sum_iters_shift=sum(info["iters_shift"]), kernel_launches=info["kernel_launches"])
         del b, x, ws
     if wl != "c5" and len(srcs) >= 4:
+        # ---- N1 (fp64, and fp32 = the MD precision)
+        for p_ in (stag.F64, stag.F32):
+            pk = packs[(p_, 18)]
+            vb = ctx.vector_bytes(p_)
+            var = "%s-18-R4" % PREC_NAME[p_]
+            a, b = ctx.upload_vectors(srcs[:4], p_), ctx.alloc(4 * vb)
+            ctx.kernel_log_reset()
+            ctx.dslash_block(pk, p_, 18, 1, 4, a, b)
+            ctx.dslash_block(pk, p_, 18, 0, 4, b, a)
+            note("stag_dslash_block R=4 x2", variant=var)
+            x, ws = ctx.alloc(4 * n * vb), ctx.alloc(ctx.cg_block_workspace_bytes(p_, n, 4))
+            bdev = ctx.upload_vectors(srcs[:4], p_)
+            stop = cfg["stops"][0] if p_ == stag.F64 else max(cfg["stops"][0], 1e-5)
+            ctx.kernel_log_reset()
+            rc, infos = ctx.mshift_cg_block(pk, p_, 18, 4, bdev, cfg["mass"], cfg["shifts"], stop, 100000, x, ws)
+            note("stag_mshift_cg_block R=4", variant=var, rc=rc, iters=[i["iters"] for i in infos],
+                 sum_iters_shift=[sum(i["iters_shift"]) for i in infos])
+            del a, b, x, ws, bdev
         pk = packs[(stag.F64, 18)]
         vb = ctx.vector_bytes(stag.F64)
-        # ---- N1
-        a, b = ctx.upload_vectors(srcs[:4], stag.F64), ctx.alloc(4 * vb)
-        ctx.kernel_log_reset()
-        ctx.dslash_block(pk, stag.F64, 18, 1, 4, a, b)
-        ctx.dslash_block(pk, stag.F64, 18, 0, 4, b, a)
-        note("stag_dslash_block R=4 x2", variant="f64-18-R4")
-        x, ws = ctx.alloc(4 * n * vb), ctx.alloc(ctx.cg_block_workspace_bytes(stag.F64, n, 4))
-        bdev = ctx.upload_vectors(srcs[:4], stag.F64)
-        ctx.kernel_log_reset()
-        rc, infos = ctx.mshift_cg_block(pk, stag.F64, 18, 4, bdev, cfg["mass"], cfg["shifts"], cfg["stops"][0], 100000, x, ws)
-        note("stag_mshift_cg_block R=4", variant="f64-18-R4", rc=rc, iters=[i["iters"] for i in infos],
-             sum_iters_shift=[sum(i["iters_shift"]) for i in infos])
-        del a, b, x, ws, bdev
         # ---- N4
         for p_ in (stag.F64, stag.F32):
             xs = ctx.upload_vectors([srcs[k % len(srcs)] for k in range(n)], p_)
@@ -863,6 +868,16 @@ def run_ours(args):
         if not args.no_block and prec != stag.F64_SPLIT:
             force, e = measure_force(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak, peak_src)
             also.append(e)
+        # ---- N1 / N4 in the MD precision (the force solves run in fp32): fp32-18 links and vectors -----
+        md_f32 = None
+        if not args.no_block and prec == stag.F64 and recon == 18 and len(srcs) >= 2:
+            pk32 = ctx.upload_gauge(U, stag.F32, 18)
+            b32, ents = measure_block(torch, stag, ctx, wl, cfg, srcs, pk32, stag.F32, 18, vh, peak, peak_src)
+            also += ents
+            f32, e = measure_force(torch, stag, ctx, wl, cfg, srcs, pk32, stag.F32, 18, vh, peak, peak_src)
+            also.append(e)
+            md_f32 = {"block": b32, "force": f32}
+            del pk32
         l2_bytes = torch.cuda.get_device_properties(local).L2_cache_size
         wset = ctx.gauge_packed_bytes(prec, recon) + (2 * nshift + 4) * vb
         iters = [i["iters"] for i in infos]
@@ -884,7 +899,7 @@ def run_ours(args):
                       "pct_of_measured": 100 * cg_gbs / peak, "equivalent_gbs": equiv_bytes_site * vh / secs / 1e9,
                       "solves": nsolves, "iters_shift_first_solve": infos[0]["iters_shift"],
                       "kernels": [norm_kernel(k) for k in step_kernels]},
-               "dslash": dslash, "solves_other_variants": solves, "block": block, "mixed": mixed, "force": force,
+               "dslash": dslash, "solves_other_variants": solves, "block": block, "mixed": mixed, "force": force, "md_f32": md_f32,
                "e2e": {"value": e2e_value, "unit": "GFLOP/s", "h2d_bytes_per_step": n6 * 8,
                        "d2h_bytes_per_step": nshift * n6 * 8, "s_per_solve": te_s / e2e_steps,
                        "call": "stag_mshift_cg_host (pinned host source in, host solutions out)"},
