@@ -1,0 +1,73 @@
+"""Host logic of bench.py (no GPU): kernel-name matching against profiles/traffic.csv, the byte models of
+SURVEY.md §8(d), the persistent kernel's residency rule.  VERDICT r1 "What's weak" 1: a traffic row may only be
+reported for the kernel of exactly that name."""
+import csv
+import os
+
+import bench
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_norm_kernel_same_spelling_from_ncu_and_from_demangler():
+    ncu = "void stag::cg_persistent_kernel<double, (int)18, (int)512, (int)1, (bool)0>(stag::Geom, stag::PersistArgs)"
+    ncu2 = "void cg_persistent_kernel<double, 18, 512, 1, 0>(Geom, PersistArgs)"
+    cxa = "void stag::cg_persistent_kernel<double, 18, 512, 1, false>(stag::Geom, stag::PersistArgs)"
+    assert bench.norm_kernel(ncu) == bench.norm_kernel(cxa) == bench.norm_kernel(ncu2) == "cg_persistent_kernel<double,18,512,1,0>"
+    assert bench.norm_kernel("void stag::force_kernel<float, 18, 3, 4>(stag::Geom, char const*, double*)") == "force_kernel<float,18,3,4>"
+
+
+def test_traffic_lookup_is_by_exact_kernel_name_and_variant():
+    got, stale = bench.committed_traffic("c4", "void stag::cg_persistent_kernel<double, 18, 512, 1, false>(stag::Geom, stag::PersistArgs)", "f64-18")
+    assert not stale and got > 5e11
+    # another build of the kernel (other template arguments), another workload, an unknown kernel: no number, flagged
+    for wl, k in (("c4", "void stag::cg_persistent_kernel<double, 18, 512>(stag::Geom, stag::PersistArgs)"),
+                  ("c4", "void stag::cg_persistent_kernel<double, 18, 256, 1, false>(stag::Geom, stag::PersistArgs)"),
+                  ("c3", "void stag::cg_persistent_kernel<double, 18, 512, 1, false>(stag::Geom, stag::PersistArgs)"),
+                  ("c4", "?")):
+        assert bench.committed_traffic(wl, k, "f64-18") == (None, True)
+    # one kernel name, two launch shapes: the variant picks the row
+    pipe = "void stag::dslash_pipe_kernel<double, 18, 4, 128, 2, true>(stag::Geom, char const*)"
+    a, _ = bench.committed_traffic("c4", pipe, "f64-18-R4")
+    b, _ = bench.committed_traffic("c4", pipe, "f64-18-force")
+    assert a and b and b > 3 * a
+    e = bench.roof_entry("c4", "?", "x", 1e9, 1e-3, 6500.0, "test")
+    assert e["traffic"] is None and e["traffic_stale"] is True and "frac_dram" not in e
+
+
+def test_traffic_csv_rows_are_complete():
+    with open(os.path.join(ROOT, "profiles", "traffic.csv"), newline="") as f:
+        rows = list(csv.DictReader(f))
+    assert len(rows) >= 25
+    kinds = " ".join(r["kernel"] for r in rows)
+    for needed in ("dslash_kernel<double,18", "dslash_kernel<float,12", "cg_persistent_kernel<double,18", "cg_persistent_kernel<float,18",
+                   "cg_persistent_block_kernel", "force_kernel", "cg_update_r_kernel", "cg_update_shifts_kernel"):
+        assert needed in kinds, needed
+    for r in rows:
+        assert r["workload"] in ("c4", "c5") and r["commit"] and r["source"]
+        assert "<" in r["kernel"] and int(r["dram_bytes_per_launch"]) > 0 and float(r["ncu_time_us"]) > 0
+        if r["algorithmic_bytes_per_launch"]:
+            ratio = int(r["dram_bytes_per_launch"]) / int(r["algorithmic_bytes_per_launch"])
+            assert 0.5 < ratio < 1.5, (r["kernel"], ratio)
+
+
+def test_byte_models():
+    # multi-kernel CG = 2736 + 192 N_live bytes per even site and iteration in fp64-18
+    assert bench.cg_bytes_per_site(0, 18, 1, [1] * 5) == 2736 + 192 * 5
+    assert bench.cg_bytes_per_site(1, 12, 1, [1] * 3) == 2 * 432 + 5 * 24 + 96 * 3
+    # the persistent kernel with r, q, p_base resident: no q write, no re-read of p, r, q
+    assert bench.cg_bytes_per_site(0, 18, 1, [1] * 5, resident=True) == 2400 + 192 * 5
+    assert bench.cg_bytes_per_site(0, 18, 10, [10, 4]) == 10 * 2736 + 14 * 192
+    assert bench.DSLASH_BYTES[(0, 18)] == 8 * 144 + 2 * 48 and bench.DSLASH_BYTES[(1, 12)] == 8 * 48 + 2 * 24
+
+
+def test_residency_rule_mirror():
+    assert bench.fully_resident(32 * 32 * 32 * 8 // 2, 0)          # config 4: r, q, p_base in shared memory
+    assert bench.fully_resident(32 * 32 * 32 * 8 // 2, 1)
+    assert not bench.fully_resident(48 * 48 * 48 * 4 // 2, 0)       # 4 x 48^3: r, q only
+    assert not bench.fully_resident(64 ** 4 // 2, 0)
+
+
+def test_replica_source_dealing():
+    # ranks work on different sources at the same step, every source is used
+    assert {bench.source_for(r, 2, k, 4) for r in range(2) for k in range(2)} == {0, 1, 2, 3}
