@@ -82,7 +82,8 @@ enum {
  * (48 significant bits).  The first stag_gauge_packed_bytes(ctx, STAG_F32, recon) bytes of a split
  * buffer ARE the STAG_F32 packed format (the b planes), so the same resident buffer also serves
  * every prec = STAG_F32 call.  Wherever a `prec` sizes or converts a VECTOR, STAG_F64_SPLIT means
- * STAG_F64.  Not accepted by the *_block calls (STAG_ERR_UNSUPPORTED). */
+ * STAG_F64.  Accepted by every call that takes a `prec` (stag_dslash_block then always runs the register-staged
+ * multi-source kernel: the cp.async ring has no split variant). */
 enum { STAG_F64 = 0, STAG_F32 = 1, STAG_F64_SPLIT = 2 };
 enum { STAG_RECON18 = 18, STAG_RECON12 = 12 };
 
@@ -274,8 +275,9 @@ int stag_mshift_cg_mixed(const stag_ctx *ctx, const void *packed_hi, int prec_hi
  *   dev_force  out, fp64 [V][4][3][3][2] (site lex, mu, row, column, re/im) — the canonical link layout;
  *              accumulate != 0 adds to it (several pseudo-fermions)
  *   workspace  stag_force_workspace_bytes (the nshift odd vectors D_oe x_i), 256-byte aligned
- * prec = STAG_F64 | STAG_F32 (the paper's choice for the force); outer products in prec, the
- * 3x3 product and projection in fp64.  Asynchronous: 2 launches (all D_oe x_i, then the force), no sync. */
+ * prec = STAG_F64 | STAG_F32 (the paper's choice for the force) | STAG_F64_SPLIT (fp64 vectors on a
+ * split-double buffer); outer products in prec, the 3x3 product and projection in fp64.  Asynchronous: the D_oe x_i
+ * launch(es), then the force kernel; no sync. */
 size_t stag_force_workspace_bytes(const stag_ctx *ctx, int prec, int nshift);
 int stag_fermion_force(const stag_ctx *ctx, const void *packed, int prec, int recon, int nshift,
                        const double *host_residues, const void *x_even, double *dev_force, int accumulate,

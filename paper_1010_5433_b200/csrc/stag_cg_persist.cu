@@ -86,7 +86,6 @@ extern "C" int stag_mshift_cg_block(const stag_ctx *ctx, const void *packed, int
     if (!ctx || !packed || !b_even || !host_shifts || !x_even || !workspace) return STAG_ERR_BADARG;
     if (!valid_prec(prec) || !valid_recon(recon)) return STAG_ERR_BADARG;
     if (nrhs < 1 || nrhs > STAG_MAX_RHS) return STAG_ERR_BADARG;
-    if (prec == STAG_F64_SPLIT) return STAG_ERR_UNSUPPORTED;
     if (nshift < 1 || nshift > STAG_MAX_SHIFTS || !(stop > 0.0) || maxiter < 0) return STAG_ERR_BADARG;
     if (y_even && !host_residues) return STAG_ERR_BADARG;
     double smin = host_shifts[0];

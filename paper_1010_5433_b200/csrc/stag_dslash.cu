@@ -59,7 +59,7 @@ dslash_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__
 // N1: R sources through one link read.  thread = one output site, ALL R sources: the 8 hopping
 // matrices are loaded into registers once and applied to the R gathered neighbours in turn, so both
 // the HBM bytes and the load-instruction count of the links are paid once per site, not per source.
-template <typename T, int RECON, int BLOCK, int RT, int R>
+template <typename T, int RECON, int BLOCK, int RT, int R, bool SPLIT = false>
 __global__ void __launch_bounds__(BLOCK, (min_ctas<BLOCK, RT>()))
 dslash_block_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ in,
                     char *__restrict__ out, const int par, const size_t stride, const int nrhs) {
@@ -69,13 +69,13 @@ dslash_block_kernel(const Geom g, const char *__restrict__ W, const char *__rest
 #pragma unroll
     for (int r = 0; r < R; ++r) ins[r] = in + (size_t)(r < nrhs ? r : 0) * stride;
     T acc[R][6];
-    dslash_site_multi<T, RECON, R>(g, W, ins, (1u << nrhs) - 1u, par, e, acc);
+    dslash_site_multi<T, RECON, R, true, SPLIT>(g, W, ins, (1u << nrhs) - 1u, par, e, acc);
 #pragma unroll
     for (int r = 0; r < R; ++r)
         if (r < nrhs) store_vec(out + (size_t)r * stride, g.Vh, e, acc[r]);
 }
 
-template <typename T, int RECON, int R>
+template <typename T, int RECON, int R, bool SPLIT = false>
 static int launch_dslash_block(const stag_ctx *ctx, const void *packed, const void *in, void *out, int par,
                                int nrhs, cudaStream_t st) {
     const Geom &g = ctx->g;
@@ -86,18 +86,18 @@ static int launch_dslash_block(const stag_ctx *ctx, const void *packed, const vo
     // registers: R accumulators + one matrix + one neighbour.  fp64: 128 per thread up to R = 2, 255 at
     // R = 4 (24 fp64 accumulators alone are 48 registers); fp32: 64 / 128.
     constexpr int RT = sizeof(T) == 8 ? (R >= 4 ? 256 : 512) : (R >= 2 ? 512 : 1024);
-    STAG_LAUNCH_K(ctx, (dslash_block_kernel<T, RECON, BLOCK, RT, R>), grid, BLOCK, 0, st, g, W,
+    STAG_LAUNCH_K(ctx, (dslash_block_kernel<T, RECON, BLOCK, RT, R, SPLIT>), grid, BLOCK, 0, st, g, W,
                   static_cast<const char *>(in), static_cast<char *>(out), par, stride, nrhs);
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
 }
 
-template <typename T, int RECON>
+template <typename T, int RECON, bool SPLIT = false>
 static int dslash_block_r(const stag_ctx *ctx, const void *packed, const void *in, void *out, int par,
                           int nrhs, cudaStream_t st) {
-    if (nrhs == 1) return launch_dslash_block<T, RECON, 1>(ctx, packed, in, out, par, nrhs, st);
-    if (nrhs == 2) return launch_dslash_block<T, RECON, 2>(ctx, packed, in, out, par, nrhs, st);
-    return launch_dslash_block<T, RECON, 4>(ctx, packed, in, out, par, nrhs, st);
+    if (nrhs == 1) return launch_dslash_block<T, RECON, 1, SPLIT>(ctx, packed, in, out, par, nrhs, st);
+    if (nrhs == 2) return launch_dslash_block<T, RECON, 2, SPLIT>(ctx, packed, in, out, par, nrhs, st);
+    return launch_dslash_block<T, RECON, 4, SPLIT>(ctx, packed, in, out, par, nrhs, st);
 }
 
 static int dslash_grid(const stag_ctx *ctx, int block, bool persistent_default) {
@@ -200,9 +200,10 @@ extern "C" int stag_dslash_block(const stag_ctx *ctx, const void *packed, int pr
     if (!ctx || !packed || !in || !out || in == out) return STAG_ERR_BADARG;
     if (!valid_prec(prec) || !valid_recon(recon) || (out_parity != 0 && out_parity != 1)) return STAG_ERR_BADARG;
     if (nrhs < 1 || nrhs > STAG_MAX_SHIFTS) return STAG_ERR_BADARG;
-    if (prec == STAG_F64_SPLIT) return STAG_ERR_UNSUPPORTED;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (ctx->opt.dslash_pipe != 0) {
+    // split-double links (N3): the register-staged kernel rebuilds a = b + c as it loads; the cp.async ring copies
+    // raw bytes into its slots and has no such variant
+    if (ctx->opt.dslash_pipe != 0 && prec != STAG_F64_SPLIT) {
         const int rc = dslash_pipe_dispatch(ctx, packed, prec, recon, out_parity, nrhs, in, out, st);
         if (rc != STAG_ERR_UNSUPPORTED) return rc;
     }
@@ -216,6 +217,9 @@ extern "C" int stag_dslash_block(const stag_ctx *ctx, const void *packed, int pr
         }
         return STAG_OK;
     }
+    if (prec == STAG_F64_SPLIT)
+        return recon == 18 ? dslash_block_r<double, 18, true>(ctx, packed, in, out, out_parity, nrhs, st)
+                           : dslash_block_r<double, 12, true>(ctx, packed, in, out, out_parity, nrhs, st);
     if (prec == STAG_F64)
         return recon == 18 ? dslash_block_r<double, 18>(ctx, packed, in, out, out_parity, nrhs, st)
                            : dslash_block_r<double, 12>(ctx, packed, in, out, out_parity, nrhs, st);

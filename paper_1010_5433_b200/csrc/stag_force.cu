@@ -26,7 +26,7 @@ struct ForceCoef { double a[STAG_MAX_SHIFTS]; };
 // The CTA's 32 x 576 contiguous output bytes leave through shared memory as full sectors.
 constexpr int kForceRow = 37;                          // 36 chunks of 16 B per site + 1 pad: conflict-free
 
-template <typename T, int RECON, int MINB, int UNR>
+template <typename T, int RECON, int MINB, int UNR, bool SPLIT = false>
 __global__ void __launch_bounds__(128, MINB)
 force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ x_even,
              const char *__restrict__ w_odd, const size_t stride, const int nshift, const ForceCoef coef,
@@ -54,13 +54,16 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
         }
         // the matrix is needed only after the shift loop: ask L2 for its lines now (no registers held), so the
         // load after the loop is an L2 hit instead of one more DRAM latency on every CTA's critical path
+        // split-double links (N3, T = double): b planes in the fp32 layout, the c planes 16 sets further on
+        const size_t set = SPLIT ? link_set_bytes<float, RECON>(Vh) : link_set_bytes<T, RECON>(Vh);
         {
-            const size_t set_ = link_set_bytes<T, RECON>(Vh);
-            const char *wl = W + (size_t)(par * 8 + 2 * mu) * set_ + (size_t)e * 16;
-            constexpr int NCH = (RECON * (int)sizeof(T) + 15) / 16;
+            const char *wl = W + (size_t)(par * 8 + 2 * mu) * set + (size_t)e * 16;
+            constexpr int NCH = (RECON * (SPLIT ? 4 : (int)sizeof(T)) + 15) / 16;
 #pragma unroll
-            for (int k = 0; k < NCH; ++k)
+            for (int k = 0; k < NCH; ++k) {
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(wl + (size_t)k * Vh * 16));
+                if (SPLIT) asm volatile("prefetch.global.L2 [%0];" ::"l"(wl + 16 * set + (size_t)k * Vh * 16));
+            }
         }
         const char *own = (par == 0 ? x_even : w_odd);     // X_i(z)
         const char *nbr = (par == 0 ? w_odd : x_even);     // X_i(z + mu)
@@ -84,8 +87,8 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
             }
         }
         T u[18];
-        const size_t set = link_set_bytes<T, RECON>(Vh);
-        load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3, policy_evict_first());
+        if constexpr (SPLIT) load_link_split<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, 16 * set, Vh, e, u, c3, policy_evict_first());
+        else load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3, policy_evict_first());
         // G = W M in fp64 (one 3x3 product per link: free next to the loads)
         double G[18];
 #pragma unroll
@@ -132,7 +135,7 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
 using namespace stag;
 
 extern "C" size_t stag_force_workspace_bytes(const stag_ctx *ctx, int prec, int nshift) {
-    if (!ctx || (prec != STAG_F64 && prec != STAG_F32) || nshift < 1 || nshift > STAG_MAX_SHIFTS) return 0;
+    if (!ctx || !valid_prec(prec) || nshift < 1 || nshift > STAG_MAX_SHIFTS) return 0;
     return align256((size_t)nshift * ctx->g.Vh * vec_bytes_per_site(prec));
 }
 
@@ -140,7 +143,7 @@ extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int p
                                   const double *host_residues, const void *x_even, double *dev_force,
                                   int accumulate, void *workspace, void *stream) {
     if (!ctx || !packed || !host_residues || !x_even || !dev_force || !workspace) return STAG_ERR_BADARG;
-    if ((prec != STAG_F64 && prec != STAG_F32) || !valid_recon(recon)) return prec == STAG_F64_SPLIT ? STAG_ERR_UNSUPPORTED : STAG_ERR_BADARG;
+    if (!valid_prec(prec) || !valid_recon(recon)) return STAG_ERR_BADARG;
     if (nshift < 1 || nshift > STAG_MAX_SHIFTS) return STAG_ERR_BADARG;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const Geom &g = ctx->g;
@@ -161,6 +164,10 @@ extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int p
     // registers (16 warps per SM) and the shift loop unrolled x2, fp32 with 3 CTAs per SM and x4
 #define STAG_FORCE(T, R, M, U) STAG_LAUNCH_K(ctx, (force_kernel<T, R, M, U>), grid, block, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate)
     if (prec == STAG_F64) { if (recon == 18) STAG_FORCE(double, 18, 4, 2); else STAG_FORCE(double, 12, 4, 2); }
+    else if (prec == STAG_F64_SPLIT) {                    // N3: fp64 vectors, a = b + c rebuilt as the matrix is loaded
+        if (recon == 18) STAG_LAUNCH_K(ctx, (force_kernel<double, 18, 4, 2, true>), grid, block, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate);
+        else STAG_LAUNCH_K(ctx, (force_kernel<double, 12, 4, 2, true>), grid, block, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate);
+    }
     else { if (recon == 18) STAG_FORCE(float, 18, 3, 4); else STAG_FORCE(float, 12, 3, 4); }
 #undef STAG_FORCE
     STAG_CUDA_OK(cudaGetLastError());

@@ -92,19 +92,12 @@ static PolishLayout polish_layout(const stag_ctx *ctx) {
     return l;
 }
 
-// D on n contiguous fp64 vectors: the N1 block kernel for native fp64 links, one launch per vector otherwise
+// D on n contiguous fp64 vectors: the N1 block kernel (native fp64 or split-double links: one read of the links)
 static int dslash_n(const stag_ctx *ctx, const void *packed, int prec, int recon, int par, int n, const char *in,
                     char *out, size_t stride, cudaStream_t st, int *launches) {
-    if (prec == STAG_F64) {
-        ++*launches;
-        return stag_dslash_block(ctx, packed, prec, recon, par, n, in, out, st);
-    }
-    for (int s = 0; s < n; ++s) {
-        ++*launches;
-        const int rc = dslash_dispatch(ctx, packed, prec, recon, in + s * stride, out + s * stride, par, st);
-        if (rc) return rc;
-    }
-    return STAG_OK;
+    (void)stride;
+    ++*launches;
+    return stag_dslash_block(ctx, packed, prec, recon, par, n, in, out, st);
 }
 
 static int polish(const stag_ctx *ctx, Slot &slot, const void *packed, int prec, int recon, const char *b, double mass,

@@ -94,6 +94,9 @@ def test_force_bad_arguments(stag):
     x = ctx.alloc(ctx.vector_bytes(0))
     ws = ctx.alloc(ctx.force_workspace_bytes(0, 1))
     with pytest.raises(stag.StagError) as e:
-        ctx.fermion_force(ctx.upload_gauge(U, stag.F64_SPLIT, 18), stag.F64_SPLIT, 18, [1.0], x, F, ws)
-    assert e.value.code == stag.ERR_UNSUPPORTED
+        ctx.fermion_force(ctx.upload_gauge(U, 0, 18), 3, 18, [1.0], x, F, ws)        # no such precision
+    assert e.value.code == stag.ERR_BADARG
+    with pytest.raises(stag.StagError) as e:
+        ctx.fermion_force(ctx.upload_gauge(U, 0, 18), 0, 18, [1.0], x, F, None)
+    assert e.value.code == stag.ERR_BADARG
     assert ctx.force_workspace_bytes(0, 0) == 0 and ctx.force_workspace_bytes(0, 33) == 0

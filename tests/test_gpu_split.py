@@ -128,12 +128,65 @@ def test_split_cg_config2_single_shift(stag):
     assert np.linalg.norm(b - oracle.apply_A(L, U, m, shifts[0], xi)) / np.linalg.norm(b) <= 1e-10
 
 
-def test_split_not_accepted_by_block_calls(stag):
-    L = (4, 4, 4, 4)
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 16, 16, 4)])
+@pytest.mark.parametrize("recon", [18, 12])
+@pytest.mark.parametrize("nrhs", [1, 2, 3, 4, 7])
+def test_split_block_dslash_matches_oracle_on_split_links(stag, L, recon, nrhs):
+    """N3 x N1: stag_dslash_block on a split-double buffer = the oracle's D applied with oracle.split_double(U),
+    every source, both parities, up to rounding; within the north_star's 1e-13 of the unsplit operator."""
+    U = si.links_haar(L, 91)
+    Us = oracle.split_double(U)
     ctx = stag.Stag(L)
-    packed = ctx.upload_gauge(si.links_haar(L, 3), stag.F64_SPLIT, 18)
-    v = ctx.alloc(2 * ctx.vector_bytes(stag.F64))
-    w = ctx.alloc(2 * ctx.vector_bytes(stag.F64))
-    with pytest.raises(stag.StagError) as e:
-        ctx.dslash_block(packed, stag.F64_SPLIT, 18, 0, 2, v, w)
-    assert e.value.code == stag.ERR_UNSUPPORTED
+    packed = ctx.upload_gauge(U, stag.F64_SPLIT, recon)
+    vb = ctx.vector_bytes(stag.F64)
+    srcs = [si.source_gaussian(L, 91, stream=1 + k) for k in range(nrhs)]
+    vin, vout = ctx.upload_vectors(srcs, stag.F64), ctx.alloc(nrhs * vb)
+    for par, ofun in ((1, oracle.dslash_oe), (0, oracle.dslash_eo)):
+        ctx.dslash_block(packed, stag.F64_SPLIT, recon, par, nrhs, vin, vout)
+        for k in range(nrhs):
+            got = ctx.download_vector(vout, stag.F64, k * vb)
+            assert rel(got, ofun(L, Us, srcs[k])) <= 5e-15
+            assert rel(got, ofun(L, U, srcs[k])) <= 1e-13
+
+
+def test_split_block_cg_equals_single_solves(stag):
+    """N3 x N1: stag_mshift_cg_block on split-double links: per source the iteration count of the single solve on
+    the same buffer and true residuals <= stop by the oracle's operator."""
+    cfg = si.get_config("c1_4x4x4x4")
+    L, U, m, shifts = cfg["L"], si.make_links(cfg), cfg["mass"], cfg["shifts"]
+    ctx = stag.Stag(L)
+    P = stag.F64_SPLIT
+    packed = ctx.upload_gauge(U, P, 18)
+    n, vb = len(shifts), ctx.vector_bytes(P)
+    srcs = [si.source_gaussian(L, 92, stream=1 + k) for k in range(3)]
+    x = ctx.alloc(3 * n * vb)
+    ws = ctx.alloc(ctx.cg_block_workspace_bytes(P, n, 3))
+    rc, infos = ctx.mshift_cg_block(packed, P, 18, 3, ctx.upload_vectors(srcs, P), m, shifts, 1e-10, 2000, x, ws)
+    assert rc == 0
+    x1, ws1 = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(P, n))
+    for s, b in enumerate(srcs):
+        rc1, i1 = ctx.mshift_cg(packed, P, 18, ctx.upload_vector(b, P), m, shifts, 1e-10, 2000, x1, ws1)
+        assert rc1 == 0 and infos[s]["iters"] == i1["iters"] and infos[s]["converged"]
+        for i, sig in enumerate(shifts):
+            xi = ctx.download_vector(x, P, (s * n + i) * vb)
+            assert np.linalg.norm(b - oracle.apply_A(L, U, m, sig, xi)) / np.linalg.norm(b) <= 1e-10
+            assert rel(xi, ctx.download_vector(x1, P, i * vb)) <= 1e-12
+
+
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 16, 16, 4)])
+@pytest.mark.parametrize("recon", [18, 12])
+def test_split_force_matches_oracle_on_split_links(stag, L, recon):
+    """N3 x N4: the fermion force read from a split-double buffer = the oracle's force with split_double(U)."""
+    import torch
+    U = si.links_haar(L, 93)
+    xs = [si.source_gaussian(L, 93, stream=1 + k) for k in range(5)]
+    residues = [0.7, -0.3, 1.9, 0.05, 2.5]
+    ctx = stag.Stag(L)
+    packed = ctx.upload_gauge(U, stag.F64_SPLIT, recon)
+    F = torch.full((ctx.V * 72,), float("nan"), dtype=torch.float64, device="cuda")
+    ws = ctx.alloc(ctx.force_workspace_bytes(stag.F64_SPLIT, 5))
+    ctx.fermion_force(packed, stag.F64_SPLIT, recon, residues, ctx.upload_vectors(xs, stag.F64), F, ws)
+    got = F.cpu().numpy().view(np.complex128).reshape(ctx.V, 4, 3, 3)
+    assert np.isfinite(got.view(np.float64)).all()
+    assert rel(got, oracle.fermion_force(L, oracle.split_double(U), residues, np.stack(xs))) <= 2e-14
+    assert rel(got, oracle.fermion_force(L, U, residues, np.stack(xs))) <= 1e-13
