@@ -21,19 +21,23 @@ struct ForceCoef { double a[STAG_MAX_SHIFTS]; };
 // made each gather of X_i(z+mu) touch 4 lines per quarter-warp and the kernel sat at 74 % of
 // l1tex__data_pipe_lsu_wavefronts; one thread per site with all 4 directions needs 144 fp64 accumulators,
 // leaves 8 warps per SM and is latency-bound (12 % warps active).  Here a thread keeps one 3x3 sum (36
-// registers), which leaves room to unroll the shift loop (fp64: x2 at 16 warps per SM; fp32: x4 at 12).
-// X_i(z) is requested by the 4 warps of a CTA (3 of the 4 hit L1).
+// registers), which leaves room to unroll the shift loop (fp64: x2 at 16 warps per SM).  X_i(z) is requested by
+// the 4 warps of a CTA (3 of the 4 hit L1).  fp32 runs with TWO links per thread (LPT below): its 36 float
+// accumulators per link leave room for two, and X_i(z) is then loaded once for both.
 // The CTA's 32 x 576 contiguous output bytes leave through shared memory as full sectors.
 constexpr int kForceRow = 37;                          // 36 chunks of 16 B per site + 1 pad: conflict-free
 
-template <typename T, int RECON, int MINB, int UNR, bool SPLIT = false>
-__global__ void __launch_bounds__(128, MINB)
+// LPT = links per thread: 1 = direction mu is the warp index (4 warps per CTA); 2 = a thread owns the links (z, mu) and
+// (z, mu + 2) and loads X_i(z) ONCE for both (2 warps per CTA): 9 instead of 12 vector loads per two links and shift.
+// The kernel is bound by the SM's load/store pipe (L1 wavefronts), not by HBM or L2 bytes.
+template <typename T, int RECON, int MINB, int UNR, bool SPLIT = false, int LPT = 1>
+__global__ void __launch_bounds__(128 / LPT, MINB)
 force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ x_even,
              const char *__restrict__ w_odd, const size_t stride, const int nshift, const ForceCoef coef,
              double *__restrict__ force, const int accumulate) {
     __shared__ double2 stage[32 * kForceRow];          // [site][mu][9 complex] (+ pad)
     __shared__ int s_lex[32];
-    const int mu = threadIdx.x >> 5, ls = threadIdx.x & 31;
+    const int wrp = threadIdx.x >> 5, ls = threadIdx.x & 31;
     // consecutive CTAs alternate parity over the same 32-site tile: the X_i one reads as X_i(z) the other reads
     // as X_i(z+mu) a moment later, out of L2 (measured: 316 -> 305 us per fp64 call)
     const int par = blockIdx.x & 1, tile = blockIdx.x >> 1;
@@ -41,22 +45,26 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
     const int Vh = g.Vh;
     if (e < Vh) {
         const Site s = site_of(g, e, par);
-        if (mu == 0) s_lex[ls] = s.lex;
+        if (wrp == 0) s_lex[ls] = s.lex;
         const int x[4] = {s.x0, s.x1, s.x2, s.x3};
-        int str = 1, phase_sum = 0;
-        for (int nu = 0; nu < mu; ++nu) { str *= g.L[nu]; phase_sum += x[nu]; }
-        const int Lmu = g.L[mu];
-        const int ef = (s.lex + str - (x[mu] == Lmu - 1 ? Lmu * str : 0)) >> 1;
-        T c3 = T(0);
-        if (RECON == 12) {
-            const T eta = (phase_sum & 1) ? T(-2) : T(2);
-            c3 = (mu == 3 && x[3] == Lmu - 1) ? -eta : eta;
-        }
-        // the matrix is needed only after the shift loop: ask L2 for its lines now (no registers held), so the
-        // load after the loop is an L2 hit instead of one more DRAM latency on every CTA's critical path
         // split-double links (N3, T = double): b planes in the fp32 layout, the c planes 16 sets further on
         const size_t set = SPLIT ? link_set_bytes<float, RECON>(Vh) : link_set_bytes<T, RECON>(Vh);
-        {
+        int ef[LPT];
+        T c3[LPT];
+#pragma unroll
+        for (int l = 0; l < LPT; ++l) {
+            const int mu = wrp + l * (4 / LPT);
+            int str = 1, phase_sum = 0;
+            for (int nu = 0; nu < mu; ++nu) { str *= g.L[nu]; phase_sum += x[nu]; }
+            const int Lmu = g.L[mu];
+            ef[l] = (s.lex + str - (x[mu] == Lmu - 1 ? Lmu * str : 0)) >> 1;
+            c3[l] = T(0);
+            if (RECON == 12) {
+                const T eta = (phase_sum & 1) ? T(-2) : T(2);
+                c3[l] = (mu == 3 && x[3] == Lmu - 1) ? -eta : eta;
+            }
+            // the matrix is needed only after the shift loop: ask L2 for its lines now (no registers held), so the
+            // load after the loop is an L2 hit instead of one more DRAM latency on every CTA's critical path
             const char *wl = W + (size_t)(par * 8 + 2 * mu) * set + (size_t)e * 16;
             constexpr int NCH = (RECON * (SPLIT ? 4 : (int)sizeof(T)) + 15) / 16;
 #pragma unroll
@@ -67,61 +75,70 @@ force_kernel(const Geom g, const char *__restrict__ W, const char *__restrict__ 
         }
         const char *own = (par == 0 ? x_even : w_odd);     // X_i(z)
         const char *nbr = (par == 0 ? w_odd : x_even);     // X_i(z + mu)
-        T m[18];
+        T m[LPT][18];
 #pragma unroll
-        for (int k = 0; k < 18; ++k) m[k] = T(0);
+        for (int l = 0; l < LPT; ++l)
+#pragma unroll
+            for (int k = 0; k < 18; ++k) m[l][k] = T(0);
 #pragma unroll UNR
         for (int i = 0; i < nshift; ++i) {
-            T a[6], b[6];
+            T a[6], b[LPT][6];
             load_vec(own + (size_t)i * stride, Vh, e, a);
-            load_vec(nbr + (size_t)i * stride, Vh, ef, b);
+#pragma unroll
+            for (int l = 0; l < LPT; ++l) load_vec(nbr + (size_t)i * stride, Vh, ef[l], b[l]);
             const T c = (T)coef.a[i];
 #pragma unroll
-            for (int r = 0; r < 3; ++r) {
-                const T br = c * b[2 * r], bi = c * b[2 * r + 1];
+            for (int l = 0; l < LPT; ++l)
 #pragma unroll
-                for (int q = 0; q < 3; ++q) {            // M[r][q] += c b_r conj(a_q)
-                    m[6 * r + 2 * q] = fma(br, a[2 * q], fma(bi, a[2 * q + 1], m[6 * r + 2 * q]));
-                    m[6 * r + 2 * q + 1] = fma(bi, a[2 * q], fma(-br, a[2 * q + 1], m[6 * r + 2 * q + 1]));
+                for (int r = 0; r < 3; ++r) {
+                    const T br = c * b[l][2 * r], bi = c * b[l][2 * r + 1];
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) {            // M[r][q] += c b_r conj(a_q)
+                        m[l][6 * r + 2 * q] = fma(br, a[2 * q], fma(bi, a[2 * q + 1], m[l][6 * r + 2 * q]));
+                        m[l][6 * r + 2 * q + 1] = fma(bi, a[2 * q], fma(-br, a[2 * q + 1], m[l][6 * r + 2 * q + 1]));
+                    }
                 }
-            }
         }
-        T u[18];
-        if constexpr (SPLIT) load_link_split<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, 16 * set, Vh, e, u, c3, policy_evict_first());
-        else load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3, policy_evict_first());
-        // G = W M in fp64 (one 3x3 product per link: free next to the loads)
-        double G[18];
 #pragma unroll
-        for (int r = 0; r < 3; ++r)
+        for (int l = 0; l < LPT; ++l) {
+            const int mu = wrp + l * (4 / LPT);
+            T u[18];
+            if constexpr (SPLIT) load_link_split<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, 16 * set, Vh, e, u, c3[l], policy_evict_first());
+            else load_link<RECON>(W + (size_t)(par * 8 + 2 * mu) * set, Vh, e, u, c3[l], policy_evict_first());
+            // G = W M in fp64 (one 3x3 product per link: free next to the loads)
+            double G[18];
 #pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                double re = 0.0, im = 0.0;
+            for (int r = 0; r < 3; ++r)
 #pragma unroll
-                for (int k = 0; k < 3; ++k) {
-                    const double ur = u[6 * r + 2 * k], ui = u[6 * r + 2 * k + 1];
-                    const double mr = m[6 * k + 2 * q], mi = m[6 * k + 2 * q + 1];
-                    re += ur * mr - ui * mi;
-                    im += ur * mi + ui * mr;
+                for (int q = 0; q < 3; ++q) {
+                    double re = 0.0, im = 0.0;
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        const double ur = u[6 * r + 2 * k], ui = u[6 * r + 2 * k + 1];
+                        const double mr = m[l][6 * k + 2 * q], mi = m[l][6 * k + 2 * q + 1];
+                        re += ur * mr - ui * mi;
+                        im += ur * mi + ui * mr;
+                    }
+                    G[6 * r + 2 * q] = re; G[6 * r + 2 * q + 1] = im;
                 }
-                G[6 * r + 2 * q] = re; G[6 * r + 2 * q + 1] = im;
-            }
-        const double eps2 = par ? -2.0 : 2.0;            // 2 eps(z)
-        const double tr_im = (G[1] + G[9] + G[17]) * (2.0 / 6.0);     // tr(G - G^dag)/6 = i * 2 Im tr G / 6
-        double2 *row = stage + ls * kForceRow + mu * 9;
+            const double eps2 = par ? -2.0 : 2.0;            // 2 eps(z)
+            const double tr_im = (G[1] + G[9] + G[17]) * (2.0 / 6.0);     // tr(G - G^dag)/6 = i * 2 Im tr G / 6
+            double2 *row = stage + ls * kForceRow + mu * 9;
 #pragma unroll
-        for (int r = 0; r < 3; ++r)
+            for (int r = 0; r < 3; ++r)
 #pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                double re = 0.5 * (G[6 * r + 2 * q] - G[6 * q + 2 * r]);
-                double im = 0.5 * (G[6 * r + 2 * q + 1] + G[6 * q + 2 * r + 1]);
-                if (r == q) im -= tr_im;
-                row[3 * r + q] = make_double2(re * eps2, im * eps2);
-            }
+                for (int q = 0; q < 3; ++q) {
+                    double re = 0.5 * (G[6 * r + 2 * q] - G[6 * q + 2 * r]);
+                    double im = 0.5 * (G[6 * r + 2 * q + 1] + G[6 * q + 2 * r + 1]);
+                    if (r == q) im -= tr_im;
+                    row[3 * r + q] = make_double2(re * eps2, im * eps2);
+                }
+        }
     }
     __syncthreads();
     // 32 sites x 36 chunks of 16 bytes; consecutive threads write consecutive chunks of one site
     const int nsite = min(32, Vh - tile * 32);
-    for (int k = threadIdx.x; k < nsite * 36; k += 128) {
+    for (int k = threadIdx.x; k < nsite * 36; k += 128 / LPT) {
         const int site = k / 36, c = k - site * 36;
         double2 v = stage[site * kForceRow + c];
         double2 *out = reinterpret_cast<double2 *>(force + (size_t)s_lex[site] * 72) + c;
@@ -160,15 +177,22 @@ extern "C" int stag_fermion_force(const stag_ctx *ctx, const void *packed, int p
     for (int i = 0; i < STAG_MAX_SHIFTS; ++i) coef.a[i] = i < nshift ? host_residues[i] : 0.0;
     const dim3 grid(2 * ((g.Vh + 31) / 32)), block(128);
     const char *W = static_cast<const char *>(packed);
-    // occupancy / unroll measured at 32^3 x 8, 16 shifts (profiles/README.md "N4"): fp64 is fastest with 128
-    // registers (16 warps per SM) and the shift loop unrolled x2, fp32 with 3 CTAs per SM and x4
+    // occupancy / unroll measured at 32^3 x 8, 16 shifts (profiles/README.md "N4"): fp64 is fastest with one link per
+    // thread, 128 registers (16 warps per SM) and the shift loop unrolled x2
 #define STAG_FORCE(T, R, M, U) STAG_LAUNCH_K(ctx, (force_kernel<T, R, M, U>), grid, block, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate)
     if (prec == STAG_F64) { if (recon == 18) STAG_FORCE(double, 18, 4, 2); else STAG_FORCE(double, 12, 4, 2); }
     else if (prec == STAG_F64_SPLIT) {                    // N3: fp64 vectors, a = b + c rebuilt as the matrix is loaded
         if (recon == 18) STAG_LAUNCH_K(ctx, (force_kernel<double, 18, 4, 2, true>), grid, block, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate);
         else STAG_LAUNCH_K(ctx, (force_kernel<double, 12, 4, 2, true>), grid, block, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate);
     }
-    else { if (recon == 18) STAG_FORCE(float, 18, 3, 4); else STAG_FORCE(float, 12, 3, 4); }
+    else {
+        // fp32: two links per thread ((z, mu) and (z, mu + 2): X_i(z) loaded once for both), 8 CTAs of 64 threads per SM,
+        // shift loop unrolled x4 — the kernel is load/store-pipe-bound and this is 9 instead of 12 vector loads per two
+        // links and shift: 119 -> 99 us at 32^3 x 8, 16 shifts.  (fp64: 72 accumulators per thread, measured slower.)
+        const dim3 block2(64);
+        if (recon == 18) STAG_LAUNCH_K(ctx, (force_kernel<float, 18, 8, 4, false, 2>), grid, block2, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate);
+        else STAG_LAUNCH_K(ctx, (force_kernel<float, 12, 8, 4, false, 2>), grid, block2, 0, st, g, W, x, w, vbytes, nshift, coef, dev_force, accumulate);
+    }
 #undef STAG_FORCE
     STAG_CUDA_OK(cudaGetLastError());
     return STAG_OK;
