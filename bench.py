@@ -128,6 +128,9 @@ def roof_entry(workload, kernel, what, alg_bytes, secs_per_launch, peak, peak_sr
         e["traffic_stale"] = True
     elif traffic:
         e["frac_dram"] = traffic / secs_per_launch / 1e9 / peak     # real HBM traffic of the capture / live time / peak
+        if e["frac_dram"] > 1.0:
+            e["frac_dram_note"] = ("the capture is cold-cache and serialised; in the live back-to-back run part of these bytes "
+                                   "(the vector the previous launch wrote) comes from L2, and a read-only stream exceeds the copy figure")
     e.update(extra)
     return e
 
