@@ -135,24 +135,35 @@ def roof_entry(workload, kernel, what, alg_bytes, secs_per_launch, peak, peak_sr
     return e
 
 
-def cg_bytes_per_site(prec, recon, iters, iters_shift, resident=False):
-    """Algorithmic bytes of one solve per even site.  Multi-kernel path, per iteration: 2 Dslash
-    + p re-read (a3) + r,q,r (a5) + r (a6), plus x_i,p_i read+write for every iteration shift i was live:
-    2D + 5 vec + 4 vec N.  resident = the persistent kernel with r, q, p_base in shared memory: q is never written
-    to memory, p, r, q are never re-read from it, and the base shift only writes p: 2D - 2 vec + 4 vec N."""
+BYTES_MODEL = {0: "2D + 5 vec + 4 vec N_live", 2: "2D + 4 vec N_live (r, q in shared memory)",
+               3: "2D - 2 vec + 4 vec N_live (r, q, p_base in shared memory)"}
+
+
+def cg_bytes_per_site(prec, recon, iters, iters_shift, resident=0):
+    """Algorithmic bytes of one solve per even site.  resident = 0, the multi-kernel path, per
+    iteration: 2 Dslash + p re-read (a3) + r,q,r (a5) + r (a6), plus x_i,p_i read+write for every iteration shift i was
+    live: 2D + 5 vec + 4 vec N.  resident = 3 (True), the persistent kernel with r, q, p_base in shared memory: q is never
+    written to memory, p, r, q are never re-read from it, and the base shift only writes p: 2D - 2 vec + 4 vec N.
+    resident = 2, r and q in shared memory but p_base in global memory (e.g. 4 x 48^3): as 3 plus the own-site read of
+    p in a3 and in the base shift's update: 2D + 4 vec N."""
     w = 4 if prec == 1 else 8
     vec = 6 * w
-    per_iter = 2 * DSLASH_BYTES[(prec, recon)] + (-2 * vec if resident else 5 * vec)
-    return iters * per_iter + sum(iters_shift) * 4 * vec
+    extra = {0: 5 * vec, 2: 0, 3: -2 * vec}[3 if resident is True else int(resident)]
+    return iters * (2 * DSLASH_BYTES[(prec, recon)] + extra) + sum(iters_shift) * 4 * vec
 
 
-def fully_resident(vh, prec, num_sms=148):
-    """Mirror of launch_persistent's residency rule (csrc/stag_cg_persist.cuh): r, q and p_base all in shared memory."""
+def resident_slices(vh, prec, num_sms=148):
+    """Mirror of launch_persistent's residency rule (csrc/stag_cg_persist.cuh): how many of r, q, p_base the persistent
+    kernel keeps in its 200 KB of shared memory (it runs with 2 or 3; below 2 the multi-kernel path is taken)."""
     w = 4 if prec == 1 else 8
     tiles = (vh + 31) // 32
     grid = min(num_sms, tiles)
     slots = 32 * ((tiles + grid - 1) // grid)
-    return 3 * slots * 6 * w <= 200 * 1024
+    return min(3, (200 * 1024) // (slots * 6 * w))
+
+
+def fully_resident(vh, prec, num_sms=148):
+    return resident_slices(vh, prec, num_sms) == 3
 
 
 class ClockSampler:
@@ -388,9 +399,10 @@ def measure_solve(torch, stag, ctx, wl, cfg, packed, prec, recon, src, vh, peak,
                                   repeats=warm + 1)
     persistent = info["kernel_launches"] == 1
     name = "%s-%d" % (PREC_NAME[prec], recon)
-    resident = persistent and fully_resident(vh, prec)
+    resident = resident_slices(vh, prec) if persistent else 0
+    resident = resident if resident >= 2 else 0        # (cg_resident_slices < 2 is a test knob: reported with the multi-kernel bytes)
     own = cg_bytes_per_site(prec, recon, info["iters"], info["iters_shift"], resident) * vh
-    equiv = cg_bytes_per_site(prec, recon, info["iters"], info["iters_shift"], False) * vh
+    equiv = cg_bytes_per_site(prec, recon, info["iters"], info["iters_shift"], 0) * vh
     d = {"rc": rc, "s_per_solve": secs, "iters": info["iters"], "us_per_iter": secs / max(info["iters"], 1) * 1e6,
          "converged": info["converged"], "stagnated": info["stagnated"], "path": "persistent" if persistent else "multi-kernel",
          "gflops_through_solve": 2 * FLOP_PER_SITE * vh * info["iters"] / secs / 1e9,
@@ -401,8 +413,7 @@ def measure_solve(torch, stag, ctx, wl, cfg, packed, prec, recon, src, vh, peak,
         e = roof_entry(wl, kern, "stag_mshift_cg %s: one launch = one %d-shift solve (%d iterations)" % (name, n, info["iters"]),
                        own, secs, peak, peak_src, variant=name, iters=info["iters"], us_per_iter=d["us_per_iter"],
                        equivalent_gbs=equiv / secs / 1e9,
-                       bytes_model="2D - 2 vec + 4 vec N_live per site and iteration (r, q, p_base in shared memory)"
-                       if resident else "2D + 5 vec + 4 vec N_live per site and iteration")
+                       bytes_model=BYTES_MODEL[resident] + " per site and iteration")
     else:
         e = None
     return d, e
@@ -795,12 +806,13 @@ def run_ours(args):
     clk = clocks.stop() if rank == 0 else None
     step_kernels = ctx.kernel_log()
     persistent = all(i["kernel_launches"] == 1 for i in infos)
-    resident = persistent and fully_resident(vh, prec)
+    resident = resident_slices(vh, prec) if persistent else 0
+    resident = resident if resident >= 2 else 0        # (cg_resident_slices < 2 is a test knob: reported with the multi-kernel bytes)
     secs, (tot_iters, own_bytes_site, equiv_bytes_site, launches) = reduce_over_ranks(
         torch, dist, world, e0.elapsed_time(e1) * 1e-3,
         [sum(i["iters"] for i in infos),
          sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"], resident) for i in infos),
-         sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"], False) for i in infos),
+         sum(cg_bytes_per_site(prec, recon, i["iters"], i["iters_shift"], 0) for i in infos),
          sum(i["kernel_launches"] for i in infos)], "cuda")
     value = 2 * FLOP_PER_SITE * vh * tot_iters / secs / 1e9
     nsolves = args.steps * world
@@ -839,7 +851,7 @@ def run_ours(args):
                               "stag_mshift_cg %s: one launch = one %d-shift solve" % (name, nshift),
                               own_bytes_site * vh / nsolves, secs / args.steps, peak, peak_src, variant=name,
                               equivalent_gbs=equiv_bytes_site * vh / secs / 1e9 / world,
-                              bytes_model=("2D - 2 vec + 4 vec N_live" if resident else "2D + 5 vec + 4 vec N_live")
+                              bytes_model=BYTES_MODEL[resident]
                               + " per even site and iteration, summed over the iterations of the solve")
         else:
             roof = None                                   # set from the Dslash sweep below (multi-kernel path)

@@ -58,6 +58,8 @@ def test_byte_models():
     # the persistent kernel with r, q, p_base resident: no q write, no re-read of p, r, q
     assert bench.cg_bytes_per_site(0, 18, 1, [1] * 5, resident=True) == 2400 + 192 * 5
     assert bench.cg_bytes_per_site(0, 18, 10, [10, 4]) == 10 * 2736 + 14 * 192
+    # r and q resident, p_base in global memory (4 x 48^3)
+    assert bench.cg_bytes_per_site(0, 18, 1, [1] * 5, resident=2) == 2496 + 192 * 5
     assert bench.DSLASH_BYTES[(0, 18)] == 8 * 144 + 2 * 48 and bench.DSLASH_BYTES[(1, 12)] == 8 * 48 + 2 * 24
 
 
@@ -66,6 +68,8 @@ def test_residency_rule_mirror():
     assert bench.fully_resident(32 * 32 * 32 * 8 // 2, 1)
     assert not bench.fully_resident(48 * 48 * 48 * 4 // 2, 0)       # 4 x 48^3: r, q only
     assert not bench.fully_resident(64 ** 4 // 2, 0)
+    assert bench.resident_slices(48 * 48 * 48 * 4 // 2, 0) == 2 and bench.resident_slices(32 * 32 * 32 * 8 // 2, 0) == 3
+    assert bench.resident_slices(64 ** 4 // 2, 0) < 2                # multi-kernel path
 
 
 def test_replica_source_dealing():
