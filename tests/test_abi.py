@@ -74,3 +74,22 @@ def test_product_does_not_import_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text
                 assert "stag_oracle" not in text
+
+
+def test_host_side_argument_checks_need_no_gpu(so_path):
+    """The error behaviour include/stag.h states for stag_ctx_create and the *_bytes calls is decided on the host,
+    before any CUDA call: bad extents -> BADARG, V >= 2^31 -> UNSUPPORTED, null handles -> 0 bytes."""
+    import ctypes as C
+    from paper_1010_5433_b200 import binding as b
+    l = b.lib()
+    h = C.c_void_p()
+    for L in ((4, 4, 4, 3), (4, 4, 4, 0), (4, -2, 4, 4), (1, 4, 4, 4)):
+        assert l.stag_ctx_create((C.c_int * 4)(*L), C.byref(h)) == b.ERR_BADARG, L
+    assert l.stag_ctx_create((C.c_int * 4)(256, 256, 256, 256), C.byref(h)) == b.ERR_UNSUPPORTED      # V = 2^32
+    assert l.stag_ctx_create(None, C.byref(h)) == b.ERR_BADARG
+    assert l.stag_ctx_create((C.c_int * 4)(4, 4, 4, 4), None) == b.ERR_BADARG
+    assert l.stag_gauge_canonical_bytes(None) == 0 and l.stag_vector_bytes(None, 0) == 0
+    assert l.stag_cg_workspace_bytes(None, 0, 4) == 0 and l.stag_force_workspace_bytes(None, 0, 4) == 0
+    for code, word in ((0, "ok"), (b.ERR_BADARG, "bad argument"), (b.ERR_UNSUPPORTED, "unsupported"),
+                       (b.ERR_NOT_SU3, "SU(3)"), (b.ERR_NOTCONV, "converge"), (b.ERR_BREAKDOWN, "breakdown")):
+        assert word in b.strerror(code)
