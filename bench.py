@@ -409,7 +409,7 @@ def measure_solve(torch, stag, ctx, wl, cfg, packed, prec, recon, src, vh, peak,
          "gbs_algorithmic": own / secs / 1e9, "pct_of_measured": 100 * own / secs / 1e9 / peak,
          "equivalent_gbs": equiv / secs / 1e9, "sum_iters_shift": sum(info["iters_shift"])}
     if persistent:
-        kern = launched(ctx, r"cg_persistent_kernel")
+        kern = launched(ctx, r"cg_persistent(_sr)?_kernel")
         e = roof_entry(wl, kern, "stag_mshift_cg %s: one launch = one %d-shift solve (%d iterations)" % (name, n, info["iters"]),
                        own, secs, peak, peak_src, variant=name, iters=info["iters"], us_per_iter=d["us_per_iter"],
                        equivalent_gbs=equiv / secs / 1e9,
@@ -847,7 +847,7 @@ def run_ours(args):
             # the whole solve is ONE kernel (stag_cg_persist.cuh): that kernel is the step.  `achieved` uses the
             # bytes THIS kernel has to move (r, q, p_base stay in shared memory); the multi-kernel formula of
             # SURVEY.md §8(d) is beside it as `equivalent_gbs`, and the real DRAM bytes of the ncu capture as `traffic`
-            roof = roof_entry(wl, next((k for k in step_kernels if "cg_persistent_kernel" in k), "?"),
+            roof = roof_entry(wl, next((k for k in step_kernels if re.search(r"cg_persistent(_sr)?_kernel", k)), "?"),
                               "stag_mshift_cg %s: one launch = one %d-shift solve" % (name, nshift),
                               own_bytes_site * vh / nsolves, secs / args.steps, peak, peak_src, variant=name,
                               equivalent_gbs=equiv_bytes_site * vh / secs / 1e9 / world,

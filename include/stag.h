@@ -129,6 +129,9 @@ const char *stag_strerror(int err);
  * its CTAs wait at the sync points of the next; 0: all at once after the base shift),
  * "cg_nbflags" (1, default: after the two stencil phases a CTA of the persistent kernel waits only for the CTAs that
  * own its neighbouring sites; 0: for all of them),
+ * "cg_single_reduction" (1, default: the single-source persistent kernel makes ONE grid-wide reduction per iteration —
+ * <p,q>, <r,q>, <q,q> and <r,r> of the current r together, ||r - alpha q||^2 = rr - 2 alpha <r,q> + alpha^2 <q,q>,
+ * rr recomputed from r every iteration; 0: two reductions, <p,q> then <r,r> of the updated r),
  * "cg_profile" (0, default; 1: see stag_cg_profile). */
 int stag_set_option(stag_ctx *ctx, const char *key, int value);
 int stag_get_option(const stag_ctx *ctx, const char *key, int *value);

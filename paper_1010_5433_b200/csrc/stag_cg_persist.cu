@@ -7,6 +7,8 @@
 
 namespace stag {
 
+int cg_persistent_sr_launch(const stag_ctx *ctx, int prec, int recon, const PersistArgs &a, cudaStream_t st);
+
 STAG_DEFINE_PERSIST_R(1)
 
 // single source: the persistent kernel is used when at least r and q fit in shared memory (all three of
@@ -41,6 +43,10 @@ int cg_persistent_dispatch(const stag_ctx *ctx, const void *packed, int prec, in
     a.flags = reinterpret_cast<unsigned int *>(ws + lay.flags);
     a.nrhs = 1;
     a.keep_mask = persist_keep_mask(ctx, prec, 1, nshift, host_shifts);
+    if (ctx->opt.cg_single_reduction) {                  // one grid-wide reduction per iteration (stag_cg_persist_sr.cuh)
+        const int rc = cg_persistent_sr_launch(ctx, prec, recon, a, st);
+        if (rc != STAG_ERR_UNSUPPORTED) return rc;
+    }
     if (prec == STAG_F64_SPLIT) return cg_persistent_launch_split(ctx, recon, 1, a, st);
     return cg_persistent_launch_r<1>(ctx, prec, recon, a, st);
 }

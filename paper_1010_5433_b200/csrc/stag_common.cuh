@@ -72,6 +72,7 @@ struct Options {
     int cg_persistent;       // 1: whole solve as one cooperative kernel when r,q,p fit in shared memory; 0: never
     int cg_l2_keep_mb;       // persistent kernel: MB of x_i, p_i (lightest shifts first) kept L2-resident (evict_last); 0: none
     int cg_fill;             // persistent kernel: 1 = deferred shift updates are worked off while waiting at sync points
+    int cg_single_reduction; // persistent kernel, single source: 1 = one grid-wide reduction per iteration (stag_cg_persist_sr.cuh)
     int cg_nbflags;          // persistent kernel: 1 = neighbour epoch flags instead of grid barriers after phases A and D
     int cg_profile;          // multi-kernel path: 1 = no graph, CUDA events around every kernel of 32 iterations (stag_cg_profile)
 };

