@@ -104,3 +104,24 @@ def test_maxiter_and_breakdown_on_the_single_reduction_kernel(stag):
     bad[3, 1] = np.nan
     rc, info, _, _ = solve(stag, ctx, packed, 0, 18, bad, 0.01, [0.0, 0.5], 1e-10, 100, 1)
     assert rc == stag.ERR_BREAKDOWN and info["breakdown"]
+
+
+@pytest.mark.parametrize("fill,nbflags", [(0, 0), (0, 1), (1, 0)])
+def test_sync_options_do_not_change_the_arithmetic(stag, fill, nbflags):
+    """cg_fill (deferred shift updates worked off in the waits) and cg_nbflags (neighbour flags instead of grid-wide
+    waits after the stencil phases) only move work and waits around: the bits of the result stay the same."""
+    L = (16, 16, 16, 4)
+    U, b = si.links_haar(L, 404), si.source_gaussian(L, 404, stream=1)
+    m, shifts = 0.05, [0.002, 0.05, 0.6, 7.0]
+    ctx = stag.Stag(L)
+    packed = ctx.upload_gauge(U, 0, 18)
+    rc0, i0, x0, k0 = solve(stag, ctx, packed, 0, 18, b, m, shifts, 1e-10, 20000, 1)
+    ctx.set_option("cg_fill", fill)
+    ctx.set_option("cg_nbflags", nbflags)
+    rc1, i1, x1, k1 = solve(stag, ctx, packed, 0, 18, b, m, shifts, 1e-10, 20000, 1)
+    ctx.set_option("cg_fill", 1)
+    ctx.set_option("cg_nbflags", 1)
+    assert "cg_persistent_sr_kernel" in k0 and "cg_persistent_sr_kernel" in k1
+    assert rc0 == 0 and rc1 == 0 and i0["iters"] == i1["iters"] and i0["rnorm2"] == i1["rnorm2"]
+    for a, c in zip(x0, x1):
+        assert np.array_equal(a, c)
