@@ -27,7 +27,15 @@ cg_persistent_block_kernel(const Geom g, const PersistArgs a) {
     constexpr int LS = NT / R;                       // streaming phases: sites per pass and source
     const int tid = threadIdx.x, G = gridDim.x, Vh = g.Vh, S = a.S;
     const int rhs = tid / LS, l0 = tid % LS;         // streaming phases: this thread's source (warp-uniform)
-    const int e0 = min(Vh, (int)blockIdx.x * S), ns = min(Vh, e0 + S) - e0;
+    // balanced contiguous ranges of 32-site tiles (no idle SM), computed once by thread 0
+    __shared__ int s_range[2];
+    if (tid == 0) {
+        const int tiles = (Vh + 31) >> 5;
+        s_range[0] = min(Vh, cta_first_tile(blockIdx.x, tiles, G) << 5);
+        s_range[1] = min(Vh, cta_first_tile(blockIdx.x + 1, tiles, G) << 5);
+    }
+    __syncthreads();
+    const int e0 = s_range[0], ns = s_range[1] - e0;
     unsigned int *bar = &a.state->ticket;
     unsigned int epoch = 0;
     double *part_pq = a.partials, *part_rr = a.partials + (size_t)R * G;
@@ -385,7 +393,7 @@ int launch_persistent_block(const stag_ctx *ctx, const PersistArgs &args, cudaSt
     const int tiles = (g.Vh + 31) / 32;
     if (grid > tiles) grid = tiles;
     PersistArgs a = args;
-    a.S = sites_per_cta(g.Vh, grid);
+    a.S = 32 * ((tiles + grid - 1) / grid);            // slots of a resident slice = the largest CTA's sites
     // residency: as many of r, q, p (in that order of bytes saved) as fit
     const size_t slice = (size_t)a.S * R * 6 * sizeof(T);
     // cg_resident_slices (test / tuning knob): cap on how many of r, q, p stay in shared memory (default 3)
