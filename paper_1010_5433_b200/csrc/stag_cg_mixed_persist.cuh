@@ -16,6 +16,9 @@
 // shifted systems ride on the base system (their residuals are taken to be zeta_i r, as in the fp64 solver);
 // what accuracy they reach is measured afterwards by stag_mshift_cg_mixed's fp64 polish, which leaves shifts
 // that are already at stop untouched.
+// One grid-wide reduction per iteration, as in stag_cg_persist_sr.cuh: <p,q>, <r,q>, <q,q> and <r,r> of the current
+// r together, ||r - alpha q||^2 by the one-step formula, phases C and D merged (0.1075 -> 0.1024 s for the
+// single-shift solve at 32^3 x 8).
 #pragma once
 
 #include "stag_cg_persist.cuh"
@@ -53,14 +56,15 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
     extern __shared__ __align__(16) unsigned char dyn[];
     __shared__ Scalars<T> sc1[1];
     __shared__ MixedExtra mx;
-    __shared__ double red[NT / 32];
+    __shared__ double red[(NT / 32) * 4];
+    __shared__ double tot[4];                        // <p,q>, <r,q>, <q,q>, <r,r> of the current r
     Scalars<T> &c = sc1[0];
 
     const int tid = threadIdx.x, G = gridDim.x, Vh = g.Vh, S = a.S;
     const int e0 = min(Vh, (int)blockIdx.x * S), ns = min(Vh, e0 + S) - e0;
     unsigned int *bar = &a.state->ticket;
     unsigned int epoch = 0;
-    double *part_pq = a.partials, *part_rr = a.partials + G;
+    double *part_pq = a.partials, *part_rr = a.partials + 3 * (size_t)G;    // [4][G]: <p,q>, <r,q>, <q,q>, <r,r>
     const CgState *st = a.state;
     const int nshift = st->nshift, base = st->base, maxiter = st->maxiter, freeze = st->freeze;
     char *p_base = a.p + (size_t)base * a.p_stride;
@@ -188,9 +192,11 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
         grid_arrive(bar);
         grid_wait(bar, ++epoch * G);
 
-        // ---- phase B (a3): q = c0 p - D_eo w, partial Re<p,q> -----------------------------------------------
+        // ---- phase B (a3): q = c0 p - D_eo w, partial Re<p,q>; then the partials of <r,q>, <q,q> and <r,r> of the
+        // current r, so that ONE grid-wide reduction gives alpha AND ||r - alpha q||^2 = rr - 2 alpha <r,q> + alpha^2
+        // <q,q> (hence beta): see stag_cg_persist_sr.cuh.  rr is recomputed from the vector r in every iteration.
         {
-            double dot = 0.0;
+            double dot[4] = {0.0, 0.0, 0.0, 0.0};
             const T c0 = c.c0;
             for (int ls = tid; ls < ns; ls += NT) {
                 const int e = e0 + ls;
@@ -200,67 +206,55 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
 #pragma unroll
                 for (int k = 0; k < 6; ++k) {
                     acc[0][k] = c0 * pv[k] - acc[0][k];
-                    dot += (double)pv[k] * (double)acc[0][k];
+                    dot[0] += (double)pv[k] * (double)acc[0][k];
                 }
                 q_s.store(ls, 0, Vh, e, acc[0]);
             }
-            cta_partials_stream<NT, 1>(dot, red, part_pq + blockIdx.x, G);
-        }
-        grid_arrive(bar);
-        grid_wait(bar, ++epoch * G);
-
-        // ---- phase C (a4, a5): alpha, theta_new_i;  r -= alpha q;  partial <r,r> ----------------------------
-        if (tid < 32) {
-            const int i = tid;
-            const double pq = grid_total(part_pq, G);
-            const double alpha = c.rr / pq;
-            const bool bad = !(pq > 0.0) || !isfinite(alpha);
-            const double k = alpha * c.beta_old / c.alpha_old;
-            __syncwarp();
-            if (!bad && i < nshift) {
-                if (c.active[i] == 2) c.active[i] = 0;
-                c.theta_new[i] = 1.0 / ((1.0 + c.delta[i] * alpha) + k * (1.0 - c.theta[i]));
-            }
-            if (i == 0) {
-                c.pq = pq;
-                if (bad) { c.breakdown = 1; c.done = 2; } else c.alpha = alpha;
-            }
-        }
-        __syncthreads();
-        if (c.done != 0) break;
-        {
-            double acc = 0.0;
-            const T na = (T)(-c.alpha);
-            for (int ls = tid; ls < ns; ls += NT) {
+            for (int ls = tid; ls < ns; ls += NT) {        // a thread re-reads the q it wrote
                 const int e = e0 + ls;
                 T rv[6], qv[6];
                 r_s.load(ls, 0, Vh, e, rv);
                 q_s.load(ls, 0, Vh, e, qv);
 #pragma unroll
                 for (int k = 0; k < 6; ++k) {
-                    rv[k] = fma(na, qv[k], rv[k]);
-                    acc += (double)rv[k] * (double)rv[k];
+                    dot[1] += (double)rv[k] * (double)qv[k];
+                    dot[2] += (double)qv[k] * (double)qv[k];
+                    dot[3] += (double)rv[k] * (double)rv[k];
                 }
-                r_s.store(ls, 0, Vh, e, rv);
             }
-            cta_partials_stream<NT, 1>(acc, red, part_rr + blockIdx.x, G);
+            cta_partials_all<NT, 4>(dot, red, part_pq + blockIdx.x, G);
         }
         grid_arrive(bar);
         grid_wait(bar, ++epoch * G);
+        if (tid < 128) {
+            const double t = grid_total(part_pq + (size_t)(tid >> 5) * G, G);
+            if ((tid & 31) == 0) tot[tid >> 5] = t;
+        }
+        __syncthreads();
 
-        // ---- phase D (a4, a7, a6): beta, zeta_i, replacement / verification trigger; x_i (fp64), p_i (fp32) ----
+        // ---- phase CD (a4, a5, a7, a6): alpha, beta, theta_i, zeta_i, replacement / verification trigger;
+        // r -= alpha q;  x_i (fp64), p_i (fp32) --------------------------------------------------------------
         if (tid < 32) {
             const int i = tid;
-            const double rr_new = grid_total(part_rr, G);
-            const double alpha = c.alpha;
-            const double beta = rr_new / c.rr;
+            const double pq = tot[0], rq = tot[1], qq = tot[2], rr = tot[3];
+            const double alpha = rr / pq;
+            const bool bad = !(pq > 0.0) || !isfinite(alpha);
+            double rr_new = fma(alpha, fma(alpha, qq, -2.0 * rq), rr);     // || r - alpha q ||^2
+            if (!bad && !(rr_new > 0.0) && rr_new == rr_new) rr_new = 0.0;
+            const double kk = alpha * c.beta_old / c.alpha_old;
+            const double beta = rr_new / rr;
             const double rel = sqrt(rr_new / c.bb);
             const int iter = c.iter + 1;
             bool live = false;
             double th = 1.0, z = 1.0;
             __syncwarp();
+            if (bad) {
+                if (i == 0) { c.pq = pq; c.breakdown = 1; c.done = 2; }
+            } else {
             if (i < nshift) {
-                th = c.theta_new[i];
+                if (c.active[i] == 2) c.active[i] = 0;
+                th = 1.0 / ((1.0 + c.delta[i] * alpha) + kk * (1.0 - c.theta[i]));
+                c.theta_new[i] = th;
                 z = c.zeta[i] * th;
                 c.zeta[i] = z;
                 c.theta[i] = th;
@@ -283,6 +277,8 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
             }
             if (i == base) { mx.a_base64 = alpha * th; c.z_base = (T)z; c.b_base = (T)(beta * th * th); }
             if (i == 0) {
+                c.pq = pq;
+                c.alpha = alpha;
                 c.nlive = __popc(m);
                 c.alpha_old = alpha;
                 c.beta_old = beta;
@@ -296,23 +292,28 @@ cg_mixed_kernel(const Geom g, const MixedArgs a) {
                                                                                  // stopped falling too — look at the true one
                 if (iter >= maxiter) { mx.ru = 1; mx.verify = 1; mx.last = 1; }
             }
+            }
         }
         __syncthreads();
+        if (c.done != 0) break;
         {
             const double ab = mx.a_base64;
-            const T zb = c.z_base, bb_ = c.b_base;
+            const T na = (T)(-c.alpha), zb = c.z_base, bb_ = c.b_base;
             for (int ls = tid; ls < ns; ls += NT) {
                 const int e = e0 + ls;
-                T rv[6], pv[6];
+                T rv[6], qv[6], pv[6];
                 double xv[6];
                 load_vec_cs(x_base, Vh, e, xv);
                 r_s.load(ls, 0, Vh, e, rv);
+                q_s.load(ls, 0, Vh, e, qv);
                 p_s.load(ls, 0, Vh, e, pv);
 #pragma unroll
                 for (int k = 0; k < 6; ++k) {
+                    rv[k] = fma(na, qv[k], rv[k]);
                     xv[k] = fma(ab, (double)pv[k], xv[k]);
                     pv[k] = fma(zb, rv[k], bb_ * pv[k]);
                 }
+                r_s.store(ls, 0, Vh, e, rv);
                 store_vec(x_base, Vh, e, xv);              // re-read by the residual replacement: keep it cached
                 if (p_s.res) p_s.s.store(ls, pv);
                 store_vec(p_base, Vh, e, pv);
