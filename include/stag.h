@@ -75,7 +75,8 @@ enum {
     STAG_ERR_CUDA = -3,         /* a CUDA runtime call or kernel launch failed                  */
     STAG_ERR_NOT_SU3 = -4,      /* recon = 12 asked for links that are not SU(3) to 1e-12       */
     STAG_ERR_NOTCONV = -5,      /* maxiter reached (or fp32 stagnation); outputs still written  */
-    STAG_ERR_BREAKDOWN = -6     /* <p,Ap> <= 0 or NaN inside CG                                 */
+    STAG_ERR_BREAKDOWN = -6,    /* <p,Ap> <= 0 or NaN inside CG                                 */
+    STAG_ERR_SCRATCH_LIMIT = -7 /* stag_fermion_force_static: needs more than STAG_FORCE_STATIC_BYTES */
 };
 /* STAG_F64_SPLIT (N3): fp64 vectors and arithmetic on links stored as TWO fp32
  * numbers per real, b = (float)a and c = (float)(a - (double)b); the kernels rebuild a' = b + c
@@ -285,6 +286,32 @@ size_t stag_force_workspace_bytes(const stag_ctx *ctx, int prec, int nshift);
 int stag_fermion_force(const stag_ctx *ctx, const void *packed, int prec, int recon, int nshift,
                        const double *host_residues, const void *x_even, double *dev_force, int accumulate,
                        void *workspace, void *stream);
+
+/* ---- the force for callers that cannot allocate device memory ------------------------------------------
+ * stag_fermion_force wants a workspace, and a workspace has to come from somewhere.  A caller may have no way to
+ * get one: a force routine plugged into another program's integrator receives the x_i and the force array and
+ * nothing else; the host program may have handed every byte of device memory to its own pool when it started, so
+ * that a cudaMalloc here fails or eats memory the host relies on; and cudaMalloc / cudaFree stall the whole device,
+ * which an MD loop that evaluates the force thousands of times on busy streams cannot pay each time.
+ * stag_fermion_force_static is stag_fermion_force without the workspace argument: same arguments otherwise, same
+ * kernels, same result; the D_oe x_i go into a fixed array of STAG_FORCE_STATIC_BYTES that is part of the library's
+ * device image.  The call itself allocates and frees nothing, on the host or on the device.
+ *   Limit      stag_force_workspace_bytes(ctx, prec, nshift) <= STAG_FORCE_STATIC_BYTES (8 MiB: e.g. 16^3 x 4 with
+ *              16 fp64 shifts = 6 MiB), else STAG_ERR_SCRATCH_LIMIT and nothing is launched.  Every GPU on which
+ *              the process uses this library carries those 8 MiB until the process exits.
+ *   Device     the context's GPU must be the current one (else STAG_ERR_BADARG): the array exists once per GPU.
+ *   First call the first call on each GPU looks the array's device address up (cudaGetSymbolAddress, which also
+ *              makes the runtime load the library's device code there) and caches it; make that call during
+ *              start-up, before any stream capture begins.  Later calls only launch.
+ *   Sharing    all calls on one GPU use the same array.  It keeps what the previous call wrote; nothing in it needs
+ *              clearing, because each call overwrites every byte it later reads.  Two calls that can overlap on
+ *              the GPU — other streams, host threads or contexts — race on it and both results are garbage:
+ *              serialise them (one stream, or events).  Calls with a caller-owned workspace are not affected. */
+#define STAG_FORCE_STATIC_BYTES (8u << 20)
+size_t stag_fermion_force_static_max_bytes(void);                   /* = STAG_FORCE_STATIC_BYTES */
+int stag_fermion_force_static(const stag_ctx *ctx, const void *packed, int prec, int recon, int nshift,
+                              const double *host_residues, const void *x_even, double *dev_force,
+                              int accumulate, void *stream);
 
 /* ---- the same calls on HOST buffers in canonical fp64 format (copies inside) --------------
  * dev_scratch: stag_host_scratch_bytes(ctx, prec, nshift) bytes of device memory

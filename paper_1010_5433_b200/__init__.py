@@ -7,5 +7,5 @@ binding without a built library raises.
 """
 from .binding import (  # noqa: F401
     F64, F32, F64_SPLIT, RECON18, RECON12, MAX_SHIFTS, MAX_RHS, OK, ERR_BADARG, ERR_UNSUPPORTED, ERR_CUDA,
-    ERR_NOT_SU3, ERR_NOTCONV, ERR_BREAKDOWN, StagError, CgInfo, PolishInfo, MixedInfo, Stag, lib, strerror, SYMBOLS,
+    ERR_NOT_SU3, ERR_NOTCONV, ERR_BREAKDOWN, ERR_SCRATCH_LIMIT, FORCE_STATIC_BYTES, StagError, CgInfo, PolishInfo, MixedInfo, Stag, lib, strerror, SYMBOLS,
 )

@@ -19,6 +19,8 @@ RECON18, RECON12 = 18, 12
 MAX_SHIFTS = 32
 MAX_RHS = 4
 OK, ERR_BADARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOT_SU3, ERR_NOTCONV, ERR_BREAKDOWN = 0, -1, -2, -3, -4, -5, -6
+ERR_SCRATCH_LIMIT = -7             # stag_fermion_force_static: problem larger than the built-in scratch
+FORCE_STATIC_BYTES = 8 << 20
 
 # every symbol include/stag.h declares
 SYMBOLS = [
@@ -31,6 +33,7 @@ SYMBOLS = [
     "stag_vector_convert", "stag_cg_polish_workspace_bytes", "stag_cg_polish",
     "stag_mshift_cg_mixed_workspace_bytes", "stag_mshift_cg_mixed",
     "stag_force_workspace_bytes", "stag_fermion_force",
+    "stag_fermion_force_static_max_bytes", "stag_fermion_force_static",
     "stag_kernel_log_reset", "stag_kernel_log", "stag_cg_profile",
 ]
 
@@ -124,6 +127,9 @@ def lib() -> C.CDLL:
     l.stag_force_workspace_bytes.argtypes = [_vp, C.c_int, C.c_int]
     l.stag_force_workspace_bytes.restype = _sz
     l.stag_fermion_force.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _dp, _vp, _vp, C.c_int, _vp, _vp]
+    l.stag_fermion_force_static_max_bytes.argtypes = []
+    l.stag_fermion_force_static_max_bytes.restype = _sz
+    l.stag_fermion_force_static.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _dp, _vp, _vp, C.c_int, _vp]
     l.stag_dslash_host.argtypes = [_vp, _vp, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp, _vp]
     l.stag_mshift_cg_host.argtypes = [_vp, _vp, C.c_int, C.c_int, _vp, C.c_double, C.c_int, _dp, _dp,
                                       C.c_double, C.c_double, C.c_int, _vp, _vp, _vp, C.POINTER(CgInfo), _vp]
@@ -330,6 +336,18 @@ class Stag:
                                       _ptr(dev_force), int(bool(accumulate)), _ptr(workspace), _stream(stream))
         if rc:
             raise StagError(rc, "stag_fermion_force")
+
+    def fermion_force_static(self, packed, prec, recon, residues, x_even, dev_force, accumulate=False, stream=None):
+        """fermion_force for callers that cannot allocate a workspace (a force callback that is handed x and F
+        only, a host program whose pool owns all device memory, a loop that must not pay cudaMalloc's device-wide
+        stall): the scratch is an 8 MiB array built into the library, one per GPU, shared by every call on that
+        GPU — so calls that might overlap on the GPU must be serialised — and problems that need more raise
+        StagError(ERR_SCRATCH_LIMIT).  The first call on a GPU also looks that array up; make it at start-up."""
+        rs = _darr(residues)
+        rc = lib().stag_fermion_force_static(self._h, _ptr(packed), prec, recon, rs[1].size, rs[0], _ptr(x_even),
+                                             _ptr(dev_force), int(bool(accumulate)), _stream(stream))
+        if rc:
+            raise StagError(rc, "stag_fermion_force_static")
 
     # ---- measurement aids
     def kernel_log_reset(self):

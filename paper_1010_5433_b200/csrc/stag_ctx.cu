@@ -89,6 +89,9 @@ extern "C" const char *stag_strerror(int err) {
         case STAG_ERR_NOT_SU3: return "links are not SU(3): 12-real reconstruction impossible";
         case STAG_ERR_NOTCONV: return "multi-shift CG did not converge";
         case STAG_ERR_BREAKDOWN: return "multi-shift CG breakdown (<p,Ap> <= 0 or NaN)";
+        case STAG_ERR_SCRATCH_LIMIT:
+            return "problem too large for the built-in scratch of stag_fermion_force_static (8 MiB): "
+                   "use stag_fermion_force with a workspace";
         default: return "unknown error";
     }
 }
