@@ -42,7 +42,12 @@ cg_persistent_sr_kernel(const Geom g, const PersistArgs a) {
     const int e0 = min(Vh, cta_first_tile(blockIdx.x, tiles, G) << 5);
     const int ns = min(Vh, cta_first_tile(blockIdx.x + 1, tiles, G) << 5) - e0;
     unsigned int *bar = &a.state->ticket;
-    double *part = a.partials;                       // [4][G]
+    // [2][4][G]: two sets of partials, used alternately by iteration parity.  There is only ONE grid-wide barrier per
+    // iteration and the syncs after phases CD and A reach a CTA's neighbours only, so a fast CTA can be in phase B of
+    // iteration n+1 while a far one has not yet summed the partials of iteration n: it must not overwrite them.  A set
+    // is rewritten two iterations later, i.e. after the next grid-wide barrier, at which every reader has arrived.
+    // The start's <b,b> sits in slot 3 of set 0, which phase B first writes in iteration 2 (same argument).
+    double *part = a.partials;
     Scalars<T> &c = sc1;
 
     CgState *st = a.state;
@@ -181,11 +186,12 @@ cg_persistent_sr_kernel(const Geom g, const PersistArgs a) {
                     dot[3] += (double)rv[k] * (double)rv[k];
                 }
             }
-            cta_partials_all<NT, 4>(dot, red, part + blockIdx.x, G);
+            cta_partials_all<NT, 4>(dot, red, part + (size_t)(gepoch & 1u) * 4 * G + blockIdx.x, G);   // gepoch = iteration
         } else {
             // phase CD: the four totals (one warp each, same order in every CTA), then every scalar of the iteration
             if (tid < 128) {
-                const double t = grid_total(part + (size_t)(tid >> 5) * G, G);
+                // the set phase B of this iteration wrote (gepoch has been incremented by the barrier since)
+                const double t = grid_total(part + (size_t)((gepoch ^ 1u) & 1u) * 4 * G + (size_t)(tid >> 5) * G, G);
                 if ((tid & 31) == 0) tot[tid >> 5] = t;
             }
             __syncthreads();
@@ -207,7 +213,11 @@ cg_persistent_sr_kernel(const Geom g, const PersistArgs a) {
                 if (!bad && !(rr_new > 0.0) && rr_new == rr_new) rr_new = 0.0; // converged to rounding
                 const double kk = alpha * c.beta_old / c.alpha_old;
                 const double beta = rr_new / rr;
-                const double rel = sqrt(rr_new / c.bb);
+                // The formula resolves rr_new only down to a few eps * rr (its three terms are all of the size of rr): a
+                // smaller value, or the clamped 0, says "below that", not "zero".  Convergence, the per-shift residuals
+                // and the freezing therefore use the bound max(rr_new, 16 eps rr); if the stop lies below it the solve
+                // goes on and the next reduction certifies the drop with the exact <r,r> (the check above).
+                const double rel = sqrt(fmax(rr_new, 16.0 * 2.220446049250313e-16 * rr) / c.bb);
                 const int iter = c.iter + 1;
                 bool live = false;
                 double th = 1.0, z = 1.0;
