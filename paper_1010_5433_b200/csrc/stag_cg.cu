@@ -232,7 +232,7 @@ static int run_multikernel(const CgLaunch<T> &L, Slot &slot, const void *b, void
     cudaEvent_t pev[kProfIters][5];
     int nprof = 0;
     if (profile) {
-        ctx->prof_iters = 0;
+        { std::lock_guard<std::mutex> lk(ctx->mu); ctx->prof_iters = 0; }
         for (int i = 0; i < kProfIters && rc == STAG_OK; ++i)
             for (int j = 0; j < 5; ++j)
                 if (cudaEventCreate(&pev[i][j]) != cudaSuccess) rc = STAG_ERR_CUDA;
@@ -306,6 +306,7 @@ static int run_multikernel(const CgLaunch<T> &L, Slot &slot, const void *b, void
                     cudaEventElapsedTime(&ms, pev[i][j], pev[i][j + 1]);
                     sum[j] += ms * 1e3;
                 }
+            std::lock_guard<std::mutex> lk(ctx->mu);         // stag_cg_profile may be called from another thread
             for (int j = 0; j < 4; ++j) ctx->prof_us[j] = sum[j] / nprof;
             ctx->prof_iters = nprof;        // (iterations run after the latch closed would count as ~0: stop is far here)
         }

@@ -183,6 +183,7 @@ extern "C" size_t stag_host_scratch_bytes(const stag_ctx *ctx, int prec, int nsh
 // ---- measurement aids -------------------------------------------------------------------------------
 extern "C" int stag_kernel_log_reset(const stag_ctx *ctx) {
     if (!ctx) return STAG_ERR_BADARG;
+    std::lock_guard<std::mutex> lk(ctx->mu);          // log_kernel of a running call takes the same lock
     ctx->nklog = 0;
     return STAG_OK;
 }
@@ -190,9 +191,16 @@ extern "C" int stag_kernel_log_reset(const stag_ctx *ctx) {
 extern "C" int stag_kernel_log(const stag_ctx *ctx, char *buf, size_t nbytes) {
     if (!ctx || !buf || nbytes == 0) return STAG_ERR_BADARG;
     std::string out;
-    for (int i = 0; i < ctx->nklog; ++i) {
+    const void *funcs[32];
+    int n = 0;
+    {
+        std::lock_guard<std::mutex> lk(ctx->mu);
+        n = ctx->nklog;
+        for (int i = 0; i < n; ++i) funcs[i] = ctx->klog[i];
+    }
+    for (int i = 0; i < n; ++i) {
         const char *mangled = nullptr;
-        if (cudaFuncGetName(&mangled, ctx->klog[i]) != cudaSuccess || !mangled) { cudaGetLastError(); continue; }
+        if (cudaFuncGetName(&mangled, funcs[i]) != cudaSuccess || !mangled) { cudaGetLastError(); continue; }
         int status = 0;
         char *dem = abi::__cxa_demangle(mangled, nullptr, nullptr, &status);
         out += (status == 0 && dem) ? dem : mangled;
@@ -201,11 +209,12 @@ extern "C" int stag_kernel_log(const stag_ctx *ctx, char *buf, size_t nbytes) {
     }
     if (out.size() + 1 > nbytes) return STAG_ERR_BADARG;
     std::memcpy(buf, out.c_str(), out.size() + 1);
-    return ctx->nklog;
+    return n;
 }
 
 extern "C" int stag_cg_profile(const stag_ctx *ctx, double us_per_launch[4], int *iterations) {
     if (!ctx || !us_per_launch || !iterations) return STAG_ERR_BADARG;
+    std::lock_guard<std::mutex> lk(ctx->mu);
     for (int j = 0; j < 4; ++j) us_per_launch[j] = ctx->prof_us[j];
     *iterations = ctx->prof_iters;
     return STAG_OK;

@@ -169,29 +169,33 @@ extern "C" int stag_gauge_pack(const stag_ctx *ctx, const double *dev_links_cano
     const Geom &g = ctx->g;
     const dim3 grid((g.Vh + 127) / 128, 16), block(128);
     char *out = static_cast<char *>(dev_packed);
-    int *flag = nullptr;
-    // recon 12: the SU(3) check writes a mapped pinned status word of a leased staging slot
+    // recon 18 needs no host staging and stays asynchronous; recon 12 runs the SU(3) check, which writes a mapped
+    // pinned status word of a staging slot leased for the duration of the call (and synchronises the stream)
+    auto launch = [&](int *flag) {
+        if (prec == STAG_F64_SPLIT) {
+            if (recon == 18) gauge_pack_kernel<SplitTag, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
+            else gauge_pack_kernel<SplitTag, 12><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
+        } else if (prec == STAG_F64) {
+            if (recon == 18) gauge_pack_kernel<double, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
+            else gauge_pack_kernel<double, 12><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
+        } else {
+            if (recon == 18) gauge_pack_kernel<float, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
+            else gauge_pack_kernel<float, 12><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
+        }
+    };
+    if (recon != 12) {
+        launch(nullptr);
+        STAG_CUDA_OK(cudaGetLastError());
+        return STAG_OK;
+    }
     SlotLease lease(ctx);
-    int *host_flag = lease.slot().pinned_flags;
-    if (recon == 12) {
-        STAG_CUDA_OK(cudaHostGetDevicePointer((void **)&flag, host_flag, 0));
-        host_flag[0] = 0;
-    }
-    if (prec == STAG_F64_SPLIT) {
-        if (recon == 18) gauge_pack_kernel<SplitTag, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
-        else gauge_pack_kernel<SplitTag, 12><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
-    } else if (prec == STAG_F64) {
-        if (recon == 18) gauge_pack_kernel<double, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
-        else gauge_pack_kernel<double, 12><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
-    } else {
-        if (recon == 18) gauge_pack_kernel<float, 18><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
-        else gauge_pack_kernel<float, 12><<<grid, block, 0, st>>>(g, dev_links_canonical, out, flag);
-    }
+    int *host_flag = lease.slot().pinned_flags, *flag = nullptr;
+    STAG_CUDA_OK(cudaHostGetDevicePointer((void **)&flag, host_flag, 0));
+    host_flag[0] = 0;
+    launch(flag);
     STAG_CUDA_OK(cudaGetLastError());
-    if (recon == 12) {
-        STAG_CUDA_OK(cudaStreamSynchronize(st));
-        if (host_flag[0] != 0) return STAG_ERR_NOT_SU3;
-    }
+    STAG_CUDA_OK(cudaStreamSynchronize(st));
+    if (host_flag[0] != 0) return STAG_ERR_NOT_SU3;
     return STAG_OK;
 }
 
