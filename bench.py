@@ -135,6 +135,86 @@ def roof_entry(workload, kernel, what, alg_bytes, secs_per_launch, peak, peak_sr
     return e
 
 
+# ---------------------------------------------------------------------------------------------
+# the ONE line the driver reads: short (< 6 KB), strict JSON, last on stdout.  Everything else the run
+# measured goes to the --detail file (round 2's 27 KB line was not parsed by the driver).
+# ---------------------------------------------------------------------------------------------
+HEADLINE_LIMIT = 6144
+# which roofline.also[] entries the headline carries, in this order (at most 10): (workload, tag)
+HEADLINE_ALSO = (("c4", "solve:f32-12"), ("c4", "block_cg:f64-18"), ("c4", "force:f64-18"), ("c4", "force:f32-18"),
+                 ("c4", "ring4:f64-18"), ("c5", "dslash:f64-18"), ("c5", "a2"), ("c5", "a3"), ("c5", "a5"), ("c5", "a6"))
+
+
+def _sig(v, n=5):
+    """floats to n significant digits (shorter line); non-finite floats to None (strict JSON)."""
+    if isinstance(v, float):
+        if v != v or v in (float("inf"), float("-inf")):
+            return None
+        return float("%.*g" % (n, v))
+    if isinstance(v, dict):
+        return {k: _sig(x, n) for k, x in v.items()}
+    if isinstance(v, (list, tuple)):
+        return [_sig(x, n) for x in v]
+    return v
+
+
+def compact_entry(e: dict) -> dict:
+    out = {k: e.get(k) for k in ("workload", "tag", "kernel", "frac", "avg_launch_us", "traffic", "frac_dram")}
+    if e.get("traffic_stale"):
+        out["traffic_stale"] = True
+    return out
+
+
+def headline(full: dict) -> dict:
+    """The driver-facing line from the full measurement dict of run_ours: the bench contract's keys, the roofline of
+    the step's dominant kernel with <= 10 compact also[] entries, the c5 (64^4) summary, cpu_baseline, e2e, clocks."""
+    keep = ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+            "vs_baseline", "dtype", "data", "config", "l2", "dslash_gflops_standalone", "cg_s_per_solve", "gpu_launches")
+    h = {k: full.get(k) for k in keep}
+    roof = full.get("roofline") or {}
+    also = roof.get("also") or []
+    picked = []
+    for wl, tag in HEADLINE_ALSO:
+        e = next((e for e in also if e.get("workload") == wl and e.get("tag") == tag), None)
+        if e is not None:
+            picked.append(compact_entry(e))
+    if not picked:                                       # other workloads / precisions: the first entries as they come
+        picked = [compact_entry(e) for e in also[:10]]
+    h["roofline"] = {k: roof.get(k) for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "frac_of_8tbs",
+                                               "algorithmic_bytes_per_launch", "avg_launch_us", "traffic", "frac_dram",
+                                               "equivalent_gbs", "bytes_model", "peak_source")}
+    if roof.get("traffic_stale"):
+        h["roofline"]["traffic_stale"] = True
+    h["roofline"]["also"] = picked[:10]
+    c5 = full.get("c5")
+    if c5 and c5.get("cg"):
+        cg = c5["cg"]
+        h["c5"] = {"workload": c5.get("workload"), "s_per_solve": cg.get("s_per_solve"), "iters": cg.get("iters"),
+                   "gbs_algorithmic": cg.get("gbs_algorithmic"),
+                   "frac": (cg.get("pct_of_measured") or 0.0) / 100.0, "timed_solves": cg.get("timed_solves"),
+                   "gflops_through_solve": cg.get("gflops_through_solve")}
+    else:
+        h["c5"] = None
+    h["cpu_baseline"] = full.get("cpu_baseline")
+    e2e = full.get("e2e") or {}
+    h["e2e"] = {k: e2e.get(k) for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step", "s_per_solve")}
+    clk = full.get("clocks")
+    if isinstance(clk, dict):
+        clk = {k: v for k, v in clk.items() if k in ("sm_mhz", "sm_max_mhz", "reasons", "samples", "power_w_max")}
+    h["clocks"] = clk
+    h["detail"] = full.get("detail_file")
+    return _sig(h)
+
+
+def headline_line(full: dict) -> str:
+    line = json.dumps(headline(full), allow_nan=False, separators=(",", ":"))
+    if len(line) >= HEADLINE_LIMIT:                     # never print a line the driver may not read: drop also[] first
+        h = headline(full)
+        h["roofline"]["also"] = h["roofline"]["also"][:4]
+        line = json.dumps(h, allow_nan=False, separators=(",", ":"))
+    return line
+
+
 BYTES_MODEL = {0: "2D + 5 vec + 4 vec N_live", 2: "2D + 4 vec N_live (r, q in shared memory)",
                3: "2D - 2 vec + 4 vec N_live (r, q, p_base in shared memory)"}
 
@@ -379,7 +459,7 @@ def dslash_variants(torch, stag, ctx, wl, U, srcs, vh, peak, peak_src, launches,
                        "pct_of_8tbs": 100 * gbs / NOMINAL_HBM_GBS, "pct_of_measured": 100 * gbs / peak,
                        "bytes_per_site": DSLASH_BYTES[(p_, r_)]}
         entries.append(roof_entry(wl, kern, "stag_dslash_oe/eo %s, %d launches ping-pong replayed as a CUDA graph" % (name, launches),
-                                  DSLASH_BYTES[(p_, r_)] * vh, s_per, peak, peak_src, variant=name,
+                                  DSLASH_BYTES[(p_, r_)] * vh, s_per, peak, peak_src, variant=name, tag="dslash:" + name,
                                   gflops=FLOP_PER_SITE * vh / s_per / 1e9))
         del pk, a, b
     del canon
@@ -411,7 +491,7 @@ def measure_solve(torch, stag, ctx, wl, cfg, packed, prec, recon, src, vh, peak,
     if persistent:
         kern = launched(ctx, r"cg_persistent(_sr)?_kernel")
         e = roof_entry(wl, kern, "stag_mshift_cg %s: one launch = one %d-shift solve (%d iterations)" % (name, n, info["iters"]),
-                       own, secs, peak, peak_src, variant=name, iters=info["iters"], us_per_iter=d["us_per_iter"],
+                       own, secs, peak, peak_src, variant=name, tag="solve:" + name, iters=info["iters"], us_per_iter=d["us_per_iter"],
                        equivalent_gbs=equiv / secs / 1e9,
                        bytes_model=BYTES_MODEL[resident] + " per site and iteration")
     else:
@@ -448,7 +528,8 @@ def measure_block(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak
         if R == 4:
             entries.append(roof_entry(wl, launched(ctx, r"dslash_(pipe|block)_kernel"),
                                       "stag_dslash_block %s, 4 sources through one link read" % name, bps * vh, s_per,
-                                      peak, peak_src, variant=name + "-R4", gflops=FLOP_PER_SITE * vh * 4 / s_per / 1e9))
+                                      peak, peak_src, variant=name + "-R4", tag="ring4:" + name,
+                                      gflops=FLOP_PER_SITE * vh * 4 / s_per / 1e9))
         del a, b
     R = min(4, len(srcs))
     n = len(cfg["shifts"])
@@ -471,7 +552,8 @@ def measure_block(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak
                  "call": "stag_mshift_cg_block (one persistent launch, links read once per Dslash for all sources)"}
     entries.append(roof_entry(wl, launched(ctx, r"cg_persistent(_block)?_kernel"),
                               "stag_mshift_cg_block %s: one launch = %d sources x %d shifts" % (name, R, n), alg, secs,
-                              peak, peak_src, variant=name + "-R%d" % R, us_per_iter=out["cg"]["us_per_iter"]))
+                              peak, peak_src, variant=name + "-R%d" % R, tag="block_cg:" + name,
+                              us_per_iter=out["cg"]["us_per_iter"]))
     return out, entries
 
 
@@ -558,14 +640,15 @@ def measure_force(torch, stag, ctx, wl, cfg, srcs, packed, prec, recon, vh, peak
          "gbs_algorithmic": gbs, "pct_of_measured": 100 * gbs / peak}
     e = roof_entry(wl, launched(ctx, r"force_kernel"),
                    "stag_fermion_force %s, %d shifts: the force kernel proper (call minus its D_oe launch of %d groups, timed alone)"
-                   % (name, n, groups), bytes_force, s_force, peak, peak_src, variant=name, us_per_call=secs * 1e6,
+                   % (name, n, groups), bytes_force, s_force, peak, peak_src, variant=name, tag="force:" + name,
+                   us_per_call=secs * 1e6,
                    call_gbs_algorithmic=gbs, call_frac=gbs / peak)
     return d, e
 
 
 def c5_section(torch, stag, args, peak, peak_src):
     """Config 5 (64^4: the largest single-GPU configuration of BASELINE.json:configs; the multi-kernel CG path):
-    the Dslash sweep, ONE timed 8-shift solve after a 32-iteration warm-up call, and the four kernels of an
+    the Dslash sweep, the MEDIAN of --c5-solves (3) timed 8-shift solves after a 32-iteration warm-up call, and the four kernels of an
     iteration timed one by one with CUDA events (option cg_profile, a separate 48-iteration call)."""
     import stag_inputs as si
     wl = "c5"
@@ -591,12 +674,14 @@ def c5_section(torch, stag, args, peak, peak_src):
     x, ws = ctx.alloc(n * vb), ctx.alloc(ctx.cg_workspace_bytes(stag.F64, n))
     ctx.kernel_log_reset()            # before the warm-up: it captures the CUDA graph the timed solve only replays
     ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], shifts, cfg["stops"][0], 32, x, ws)          # warm-up: 32 iterations
-    secs, (rc, info) = timed_call(torch, lambda: ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], shifts, cfg["stops"][0],
-                                                               100000, x, ws), repeats=1)
+    runs = [timed_call(torch, lambda: ctx.mshift_cg(p64, stag.F64, 18, b, cfg["mass"], shifts, cfg["stops"][0],
+                                                    100000, x, ws), repeats=1) for _ in range(max(1, args.c5_solves))]
+    secs, (rc, info) = sorted(runs, key=lambda t: t[0])[len(runs) // 2]          # the median solve
     alg = cg_bytes_per_site(0, 18, info["iters"], info["iters_shift"]) * vh
     out["cg"] = {"rc": rc, "s_per_solve": secs, "iters": info["iters"], "us_per_iter": secs / max(info["iters"], 1) * 1e6,
                  "gflops_through_solve": 2 * FLOP_PER_SITE * vh * info["iters"] / secs / 1e9,
                  "gbs_algorithmic": alg / secs / 1e9, "pct_of_measured": 100 * alg / secs / 1e9 / peak,
+                 "timed_solves": len(runs), "s_per_solve_all": [t[0] for t in runs],
                  "kernel_launches": info["kernel_launches"], "iters_shift": info["iters_shift"],
                  "path": "multi-kernel (4 launches per iteration, CUDA-graph replay)"}
     names = ctx.kernel_log()
@@ -617,7 +702,7 @@ def c5_section(torch, stag, args, peak, peak_src):
                                           (k_a5, "a5: r -= alpha q, <r,r>", 3 * vec, us[2]),
                                           (k_a6, "a6: all-shift update, %d live shifts" % n, vec + 4 * vec * n, us[3])):
             entries.append(roof_entry(wl, kern, "stag_mshift_cg f64-18 multi-kernel path, " + what + " (CUDA events around each launch)",
-                                      bytes_site * vh, t * 1e-6, peak, peak_src, variant="f64-18"))
+                                      bytes_site * vh, t * 1e-6, peak, peak_src, variant="f64-18", tag=what[:2]))
     del x, ws, b
     # ---- Dslash sweep
     table, ents = dslash_variants(torch, stag, ctx, wl, U, srcs, vh, peak, peak_src, args.dslash_launches,
@@ -900,11 +985,11 @@ def run_ours(args):
         out = {"metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": secs * 1e3 / args.steps, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.prec == "f32" else "f64", "data": "synthetic",
-               "config": dict(workload_config(cfg, wl, prec, recon),
-                              l2="working set (2 link sets + %d vectors) = %.0f MB %s the %.0f MB L2%s"
-                                 % (2 * nshift + 4, wset / 1e6, "exceeds" if wset > l2_bytes else "FITS in", l2_bytes / 1e6,
-                                    "; no flush between steps" if wset > l2_bytes else
-                                    ": an L2-resident run, not held to the HBM roofline")),
+               "config": workload_config(cfg, wl, prec, recon),      # the same keys in both arms (the reference arm's too)
+               "l2": "working set (2 link sets + %d vectors) = %.0f MB %s the %.0f MB L2%s"
+                     % (2 * nshift + 4, wset / 1e6, "exceeds" if wset > l2_bytes else "FITS in", l2_bytes / 1e6,
+                        "; no flush between steps" if wset > l2_bytes else
+                        ": an L2-resident run, not held to the HBM roofline"),
                "dslash_gflops_through_solve": value,
                "dslash_gflops_standalone": dslash[name]["gflops"],
                "cg_s_per_solve": secs / args.steps,
@@ -935,12 +1020,27 @@ def run_ours(args):
         # ---- cpu_baseline: the oracle on this box's host cores, bounded sample (rank 0, N = 1 only) ----
         cpu = None
         if world == 1 and not args.no_cpu_baseline:
-            g, s_it, m = oracle_sample(cfg, U, srcs[0], 12.0)
+            g, s_it, m = oracle_sample(cfg, U, srcs[0], 10.0)
             cpu = {"value": g, "unit": "GFLOP/s", "cores": 1, "kind": "oracle",
                    "sample": "%d oracle multi-shift CG iterations (maxiter=%d) of the same %d-shift solve, %.3f s/iteration"
                              % (m, m, nshift, s_it)}
+            # the same oracle, same sample rule, on every host core (its OpenMP mode: chunk-ordered deterministic
+            # reductions, bit-equal to one thread — tests/test_oracle_pins.py), BASELINE.md §5
+            ncores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+            if ncores > 1:
+                ga, sa, ma = oracle_sample(cfg, U, srcs[0], 6.0, threads=ncores)
+                cpu["all_cores"] = {"value": ga, "cores": ncores, "iterations": ma, "s_per_iteration": sa}
         out["cpu_baseline"] = cpu
-        print(json.dumps(out))
+        # every measurement of the run -> the detail file; stdout carries ONE short line, last
+        try:
+            os.makedirs(os.path.dirname(os.path.abspath(args.detail)), exist_ok=True)
+            with open(args.detail, "w") as f:
+                json.dump(_sig(out, 9), f, allow_nan=False)
+            out["detail_file"] = os.path.relpath(args.detail, ROOT)
+        except OSError:
+            out["detail_file"] = None
+        sys.stdout.flush()
+        print(headline_line(out), flush=True)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -961,6 +1061,9 @@ def main():
     ap.add_argument("--no-block", action="store_true",
                     help="skip the other storage variants' solves and the N1 multi-source, N2/N3 mixed-precision, N4 force measurements")
     ap.add_argument("--no-c5", action="store_true", help="skip the 64^4 section of the default (c4, f64-18, 1 GPU) run")
+    ap.add_argument("--c5-solves", type=int, default=3, help="timed 64^4 solves of that section (the median is reported)")
+    ap.add_argument("--detail", default=os.path.join(ROOT, "gpurun_out", "bench_detail.json"),
+                    help="file that receives every measurement of the run (stdout carries the one short headline line)")
     ap.add_argument("--ref-seconds", type=float, default=150.0,
                     help="--impl reference: total oracle time budget over all steps")
     ap.add_argument("--dslash-only", action="store_true", help="Dslash bandwidth sweep only (no CG)")

@@ -75,3 +75,90 @@ def test_residency_rule_mirror():
 def test_replica_source_dealing():
     # ranks work on different sources at the same step, every source is used
     assert {bench.source_for(r, 2, k, 4) for r in range(2) for k in range(2)} == {0, 1, 2, 3}
+
+
+def _canned_full_measurement():
+    """A full measurement dict of the shape run_ours builds, with the things that made round 2's line 27 KB: 25
+    also[] entries that each repeat long `what` / `peak_source` / note strings, and whole per-section objects."""
+    long = "x" * 220
+
+    def entry(wl, tag, kernel, frac):
+        return {"bound": "hbm", "kernel": kernel, "what": long, "workload": wl, "tag": tag, "achieved": 6455.3 * frac,
+                "peak": 6455.3, "unit": "GB/s", "frac": frac, "peak_source": "measured (MEASURED_PEAKS.json)",
+                "frac_of_8tbs": 0.8 * frac, "algorithmic_bytes_per_launch": 163577856, "avg_launch_us": 22.812345678,
+                "traffic": 160977728, "frac_dram": 0.98123456789, "frac_dram_note": long}
+
+    also = []
+    for wl in ("c4", "c5"):
+        for v in ("f64-18", "f64-12", "f32-18", "f32-12", "f64split-18", "f64split-12"):
+            also.append(entry(wl, "dslash:" + v, "dslash_kernel<double,18,128,0,512,0>", 1.08))
+    for v in ("f64-12", "f32-18", "f32-12"):
+        also.append(entry("c4", "solve:" + v, "cg_persistent_sr_kernel<float,12,1024,0>", 0.85))
+    for v in ("f64-18", "f32-18"):
+        also.append(entry("c4", "ring4:" + v, "dslash_pipe_kernel<double,18,4,128,2,1>", 0.92))
+        also.append(entry("c4", "block_cg:" + v, "cg_persistent_block_kernel<double,18,512,4,0>", 0.86))
+        also.append(entry("c4", "force:" + v, "force_kernel<double,18,4,2,0,1>", 0.51))
+    for t in ("a2", "a3", "a5", "a6"):
+        also.append(entry("c5", t, "cg_update_shifts_kernel<double,256>", 0.97))
+    roof = entry("c4", None, "cg_persistent_sr_kernel<double,18,512,0>", 0.992)
+    roof.update(equivalent_gbs=7067.0, bytes_model=bench.BYTES_MODEL[3] + " per even site and iteration", also=also)
+    big = {"k%d" % i: {"us": 1.0 * i, "note": long} for i in range(40)}
+    return {"metric": bench.METRIC, "value": 2193.8123456, "unit": "GFLOP/s", "n_gpus": 1, "steps": 20, "warmup": 5,
+            "ms_per_step": 203.5, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": "c4_32x32x32x8: ...", "prec": "f64", "recon": 18, "nshift": 16,
+                                            "parallelism": "replicas"},
+            "l2": "working set exceeds L2; no flush", "dslash_gflops_standalone": 3281.0, "cg_s_per_solve": 0.2035,
+            "cg": big, "dslash": big, "block": big, "mixed": big, "force": big, "md_f32": big, "solves_other_variants": big,
+            "e2e": {"value": 2172.0, "unit": "GFLOP/s", "h2d_bytes_per_step": 6291456, "d2h_bytes_per_step": 100663296,
+                    "s_per_solve": 0.2055, "call": long},
+            "gpu_launches": 20, "options": [], "pack_ms": 1.0, "input_gen_s": 3.0,
+            "clocks": {"sm_mhz": 1807.0, "sm_max_mhz": 1965.0, "reasons": ["sw_power_cap"], "samples": 40},
+            "c5": {"workload": "c5_64x64x64x64", "cg": {"s_per_solve": 8.14, "iters": 2006, "gbs_algorithmic": 6674.0,
+                                                         "pct_of_measured": 103.2, "timed_solves": 3,
+                                                         "gflops_through_solve": float("nan")}, "dslash": big},
+            "roofline": roof,
+            "cpu_baseline": {"value": 1.49, "unit": "GFLOP/s", "cores": 1, "kind": "oracle", "sample": "74 iterations",
+                             "all_cores": {"value": 20.1, "cores": 32, "iterations": 200, "s_per_iteration": 0.007}},
+            "detail_file": "gpurun_out/bench_detail.json"}
+
+
+def test_headline_line_is_short_strict_json_with_the_contract_keys():
+    """the driver parsed nothing from a 27 KB line.  The line bench.py prints must stay under 6 KB, be
+    strict JSON (no NaN / Infinity) and carry the contract's keys; the bulk goes to the --detail file."""
+    import json
+    full = _canned_full_measurement()
+    assert len(json.dumps(full)) > 20000                     # the canned input is as bulky as round 2's line
+    line = bench.headline_line(full)
+    assert "\n" not in line and len(line) < bench.HEADLINE_LIMIT == 6144
+
+    def no_constants(name):
+        raise ValueError("non-strict JSON constant " + name)
+    h = json.loads(line, parse_constant=no_constants)
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "clocks", "gpu_launches", "c5"):
+        assert k in h, k
+    assert h["value"] > 0 and h["n_gpus"] == 1 and h["steps"] == 20 and h["warmup"] == 5
+    assert "l2" not in h["config"] and sorted(h["config"]) == ["nshift", "parallelism", "prec", "recon", "workload"]
+    r = h["roofline"]
+    for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "frac_dram", "frac_of_8tbs",
+              "algorithmic_bytes_per_launch", "avg_launch_us", "equivalent_gbs", "bytes_model"):
+        assert k in r, k
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-3
+    assert 1 <= len(r["also"]) <= 10
+    assert [(e["workload"], e["tag"]) for e in r["also"]] == list(bench.HEADLINE_ALSO)
+    for e in r["also"]:
+        assert set(e) <= {"workload", "tag", "kernel", "frac", "avg_launch_us", "traffic", "frac_dram", "traffic_stale"}
+    assert h["c5"]["timed_solves"] == 3 and h["c5"]["gflops_through_solve"] is None      # the NaN became null
+    assert abs(h["c5"]["frac"] - 1.032) < 1e-6
+    assert h["cpu_baseline"]["cores"] == 1 and h["cpu_baseline"]["all_cores"]["cores"] == 32
+    assert h["e2e"]["h2d_bytes_per_step"] == 6291456 and "call" not in h["e2e"]
+    assert h["clocks"]["reasons"] == ["sw_power_cap"]
+
+
+def test_both_arms_describe_the_workload_with_the_same_config():
+    import stag_inputs as si
+    cfg = si.get_config(bench.WORKLOADS["c4"])
+    a = bench.workload_config(cfg, "c4", 0, 18)
+    assert sorted(a) == ["nshift", "parallelism", "prec", "recon", "workload"]
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert src.count('"config": workload_config(cfg,') == 2          # run_reference and run_ours, nothing added to either
