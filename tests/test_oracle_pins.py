@@ -457,3 +457,50 @@ def test_P10_force_is_traceless_antihermitian_and_gauge_covariant():
     # linear in the residues, quadratic in x
     assert rel(oracle.fermion_force(L, U, [2.0, 1.0], x), 2 * F) <= 1e-14
     assert rel(oracle.fermion_force(L, U, residues, 3 * x), 9 * F) <= 1e-14
+
+
+# ---- the threaded mode of the oracle (oracle.set_threads(k > 1)) -----------------------------------------------
+# Every full-size GPU parity test runs the oracle on several host cores (tests/test_gpu_fullsize.py and others call
+# oracle.set_threads(8..32)).  SURVEY.md §8(d): "no algorithmic change, chunk-ordered deterministic reductions".
+# The pin: for any thread count the results are BIT-equal to the one-thread oracle, which pins P1-P10 above hold.
+@pytest.mark.parametrize("L", [(4, 4, 4, 4), (6, 4, 2, 8)])
+def test_P11_threaded_oracle_is_bit_equal_to_one_thread(L):
+    U = si.links_haar(L, 111)
+    b = si.source_gaussian(L, 111, stream=1)
+    xs = np.stack([si.source_gaussian(L, 111, stream=2 + k) for k in range(3)])
+    mass, shifts, residues = 0.25, [0.0, 0.3, 2.0], [0.7, -0.3, 1.9]
+
+    def everything():
+        w = oracle.dslash_oe(L, U, b)
+        cg = oracle.mshift_cg(L, U, b, mass, shifts, 1e-10, 3000, want_history=True)
+        pol = oracle.cg_polish(L, U, b, mass, shifts[1], 0.5 * cg["x"][1], 1e-12, 3000)
+        return dict(w=w, q=oracle.dslash_eo(L, U, w), A=oracle.apply_A(L, U, mass, 0.3, b), x=cg["x"], zeta=cg["zeta"],
+                    r=cg["r"], hist=cg["rr_hist"], iters=cg["iters"], rc=cg["rc"], px=pol["x"], piters=pol["iters"],
+                    pres0=pol["res0"], F=oracle.fermion_force(L, U, residues, xs), n2=oracle.norm2(b))
+    try:
+        oracle.set_threads(1)
+        want = everything()
+        assert want["rc"] == 0 and want["iters"] > 10
+        for k in (2, 5, 8):
+            oracle.set_threads(k)
+            got = everything()
+            for key, v in want.items():
+                if isinstance(v, np.ndarray):
+                    assert np.array_equal(got[key], v), (k, key)
+                else:
+                    assert got[key] == v, (k, key)
+    finally:
+        oracle.set_threads(1)
+
+
+def test_P11_norm2_is_the_plain_sum_of_squares():
+    # integers: every partial sum is exact, so any summation order must give n(n+1)(2n+1)/6 exactly
+    n = 3 * 128
+    v = (np.arange(1, 2 * n + 1, 2) + 1j * np.arange(2, 2 * n + 2, 2)).reshape(128, 3)
+    m = 2 * n
+    assert oracle.norm2(v) == m * (m + 1) * (2 * m + 1) // 6
+    b = si.source_gaussian((4, 4, 4, 4), 5)
+    assert abs(oracle.norm2(b) - np.vdot(b, b).real) <= 1e-13 * oracle.norm2(b)
+    # and it is the <b,b> the CG starts from: rr_hist[0]
+    U = si.links_haar((4, 4, 4, 4), 5)
+    assert oracle.mshift_cg((4, 4, 4, 4), U, b, 0.1, [0.0], 1e-3, 5, want_history=True)["rr_hist"][0] == oracle.norm2(b)
