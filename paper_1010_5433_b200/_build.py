@@ -36,8 +36,6 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False, timers: bool = False) -> str:
     """timers=True: the per-phase-timer build of the persistent CG (csrc/stag_cg_persist.cuh), a separate .so."""
-    if os.environ.get("STAG_SO"):                  # experimental build: STAG_SO=<path> STAG_NVCC_EXTRA="-D..."
-        return _build(os.environ["STAG_SO"], ["-DSTAG_PHASE_TIMERS=" + os.environ.get("STAG_PHASE_TIMERS", "1")] if timers else [], verbose)
     if timers:
         return _build(SO_TIMERS, ["-DSTAG_PHASE_TIMERS=" + os.environ.get("STAG_PHASE_TIMERS", "1")], verbose)
     if not force and not stale():
@@ -49,8 +47,7 @@ def _build(SO: str, defines: list[str], verbose: bool) -> str:
     from concurrent.futures import ThreadPoolExecutor
     nvcc = os.environ.get("NVCC", "nvcc")
     os.makedirs(OBJ, exist_ok=True)
-    # STAG_NVCC_EXTRA: extra nvcc flags for experiments, e.g. "-DSTAG_SOMETHING -maxrregcount=..."
-    extra = (["-Xptxas", "-v"] if verbose else []) + defines + os.environ.get("STAG_NVCC_EXTRA", "").split()
+    extra = (["-Xptxas", "-v"] if verbose else []) + defines
 
     def compile_one(src: str) -> str:          # one translation unit per worker: seconds, not a minute
         obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".%d.o" % os.getpid())

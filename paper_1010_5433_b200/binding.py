@@ -11,8 +11,6 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 SO = os.path.join(HERE, "libstag_b200.so")
 if os.environ.get("STAG_PHASE_TIMERS") == "1":     # per-phase-timer build of the persistent CG (see _build.py)
     SO = os.path.join(HERE, "libstag_b200_timers.so")
-if os.environ.get("STAG_SO"):                      # an experimental build of the same sources (absolute path)
-    SO = os.environ["STAG_SO"]
 
 F64, F32, F64_SPLIT = 0, 1, 2      # F64_SPLIT (N3): split-double links, fp64 vectors
 RECON18, RECON12 = 18, 12

@@ -1,6 +1,6 @@
 """Out-of-bounds writes: every output / workspace buffer of the main calls is carved out of a larger allocation
 with 4 KB guard zones on both sides, filled with a pattern; after the call the guards must be untouched and the
-*_bytes() sizes the header promises must have been enough.  (compute-sanitizer is not available on the GPU pool.)
+*_bytes() sizes the header promises must have been enough.  (compute-sanitizer is closed on the GPU pool: profiles/r3_sanitizer_unavailable.txt holds the command and the pool's refusal.)
 Ragged lattices, so that partial warps / CTAs / per-SM slices are exercised."""
 import numpy as np
 import pytest
