@@ -81,6 +81,27 @@ def norm_kernel(name: str) -> str:
     return n
 
 
+_CSRC_SHA = None
+
+
+def csrc_sha() -> str:
+    """Fingerprint of the CUDA sources the library is built from (csrc/*.cu, *.cuh, include/stag.h): a traffic.csv
+    row is evidence for the kernels of exactly these sources.  (No git on the GPU box: the snapshot has no .git.)"""
+    global _CSRC_SHA
+    if _CSRC_SHA is None:
+        import glob
+        import hashlib
+        h = hashlib.sha256()
+        csrc = os.path.join(ROOT, "paper_1010_5433_b200", "csrc")
+        for f in sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh"))) + \
+                [os.path.join(ROOT, "include", "stag.h")]:
+            h.update(os.path.basename(f).encode() + b"\0")
+            with open(f, "rb") as fh:
+                h.update(fh.read())
+        _CSRC_SHA = h.hexdigest()[:12]
+    return _CSRC_SHA
+
+
 def load_traffic():
     import csv
     rows = []
@@ -101,14 +122,16 @@ def committed_traffic(workload: str, kernel: str, variant: str = ""):
     """(dram bytes per launch, stale flag).  The row must be for this workload and for a kernel of exactly the
     name the run launched (`kernel` comes from stag_kernel_log); a capture of another build of the kernel — other
     template arguments — is NOT returned: (None, True).  `variant` disambiguates rows of one kernel name whose
-    traffic depends on run-time arguments (e.g. the number of sources of the block kernel)."""
+    traffic depends on run-time arguments (e.g. the number of sources of the block kernel).  A row captured from
+    other sources than the ones in the tree (its `csrc_sha` differs from csrc_sha(): the kernel may have been
+    rewritten under the same name) is returned WITH the stale flag."""
     global _TRAFFIC
     if _TRAFFIC is None:
         _TRAFFIC = load_traffic()
     k = norm_kernel(kernel)
     for row in _TRAFFIC:
         if row["workload"] == workload and row["_k"] == k and (not variant or row.get("variant", "") == variant):
-            return int(row["dram_bytes_per_launch"]), False
+            return int(row["dram_bytes_per_launch"]), row.get("csrc_sha", "") != csrc_sha()
     return None, True
 
 
@@ -126,7 +149,7 @@ def roof_entry(workload, kernel, what, alg_bytes, secs_per_launch, peak, peak_sr
          "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": secs_per_launch * 1e6, "traffic": traffic}
     if stale:
         e["traffic_stale"] = True
-    elif traffic:
+    if traffic:
         e["frac_dram"] = traffic / secs_per_launch / 1e9 / peak     # real HBM traffic of the capture / live time / peak
         if e["frac_dram"] > 1.0:
             e["frac_dram_note"] = ("the capture is cold-cache and serialised; in the live back-to-back run part of these bytes "
@@ -790,7 +813,7 @@ def ncu_pass(args, torch, stag, ctx, cfg, U, srcs, vh):
         rc, info = ctx.mshift_cg_mixed(pk, stag.F64, 18, packs[(stag.F64_SPLIT, 18)], 18, b, cfg["mass"], cfg["shifts"][:1],
                                        cfg["stops"][0], 100000, x, ws)
         note("stag_mshift_cg_mixed 1 shift", variant="f64-18+f32-18", rc=rc, route=info["route"], iters=info["inner"]["iters"])
-    print(json.dumps({"ncu_pass": WORKLOADS[wl], "sequence": seq}))
+    print(json.dumps({"ncu_pass": WORKLOADS[wl], "csrc_sha": csrc_sha(), "vh": vh, "nshift": n, "sequence": seq}))
     return 0
 
 

@@ -33,6 +33,15 @@ def test_traffic_lookup_is_by_exact_kernel_name_and_variant():
     assert a and b and b > 3 * a
     e = bench.roof_entry("c4", "?", "x", 1e9, 1e-3, 6500.0, "test")
     assert e["traffic"] is None and e["traffic_stale"] is True and "frac_dram" not in e
+    # a row captured from other sources than the tree's is reported, flagged
+    saved = bench._TRAFFIC
+    try:
+        bench._TRAFFIC = [dict(r, csrc_sha="0" * 12) for r in saved]
+        got, stale = bench.committed_traffic("c4", pipe, "f64-18-R4")
+        assert got == a and stale
+        assert bench.roof_entry("c4", pipe, "x", 1e9, 1e-3, 6500.0, "test", variant="f64-18-R4")["traffic_stale"] is True
+    finally:
+        bench._TRAFFIC = saved
 
 
 def test_traffic_csv_rows_are_complete():
@@ -45,6 +54,9 @@ def test_traffic_csv_rows_are_complete():
         assert needed in kinds, needed
     for r in rows:
         assert r["workload"] in ("c4", "c5") and r["commit"] and r["source"]
+        # evidence of exactly the CUDA sources in the tree (a kernel rewritten under the same name
+        # must not keep its old traffic row): after any change under csrc/ the ncu passes have to be re-captured
+        assert r["csrc_sha"] == bench.csrc_sha(), "profiles/traffic.csv was captured from other CUDA sources: re-capture"
         assert "<" in r["kernel"] and int(r["dram_bytes_per_launch"]) > 0 and float(r["ncu_time_us"]) > 0
         if r["algorithmic_bytes_per_launch"]:
             ratio = int(r["dram_bytes_per_launch"]) / int(r["algorithmic_bytes_per_launch"])
