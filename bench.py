@@ -141,12 +141,39 @@ def launched(ctx, pattern: str) -> str:
     return names[0] if names else "?"
 
 
+_READ_PEAK = None
+
+
+def read_stream_gbs(torch, nbytes: int = 4 << 30, repeats: int = 10):
+    """A second yardstick beside MEASURED_PEAKS.json's copy bandwidth (read-dominated kernels exceed the
+    copy figure, which mixes reads and writes): GB/s of a READ-ONLY stream over 4 GiB, best of `repeats`, timed with
+    CUDA events.  The probe is a torch reduction (a library kernel used as a ruler only, as the driver's copy_ is);
+    nothing of the product path runs in it.  Measured once per process."""
+    global _READ_PEAK
+    if _READ_PEAK is None:
+        a = torch.ones(nbytes // 4, dtype=torch.float32, device="cuda")
+        best = float("inf")
+        for _ in range(repeats + 2):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            a.sum()
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1) * 1e-3)
+        del a
+        torch.cuda.empty_cache()
+        _READ_PEAK = nbytes / best / 1e9
+    return _READ_PEAK
+
+
 def roof_entry(workload, kernel, what, alg_bytes, secs_per_launch, peak, peak_src, variant="", **extra):
     gbs = alg_bytes / secs_per_launch / 1e9
     traffic, stale = committed_traffic(workload, kernel, variant)
     e = {"bound": "hbm", "kernel": norm_kernel(kernel), "what": what, "workload": workload, "achieved": gbs, "peak": peak,
          "unit": "GB/s", "frac": gbs / peak, "peak_source": peak_src, "frac_of_8tbs": gbs / NOMINAL_HBM_GBS,
          "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_us": secs_per_launch * 1e6, "traffic": traffic}
+    if _READ_PEAK:
+        e["frac_read"] = gbs / _READ_PEAK                  # against the read-only stream (never the headline `frac`)
     if stale:
         e["traffic_stale"] = True
     if traffic:
@@ -182,7 +209,7 @@ def _sig(v, n=5):
 
 
 def compact_entry(e: dict) -> dict:
-    out = {k: e.get(k) for k in ("workload", "tag", "kernel", "frac", "avg_launch_us", "traffic", "frac_dram")}
+    out = {k: e.get(k) for k in ("workload", "tag", "kernel", "frac", "frac_read", "avg_launch_us", "traffic", "frac_dram")}
     if e.get("traffic_stale"):
         out["traffic_stale"] = True
     return out
@@ -205,7 +232,8 @@ def headline(full: dict) -> dict:
         picked = [compact_entry(e) for e in also[:10]]
     h["roofline"] = {k: roof.get(k) for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "frac_of_8tbs",
                                                "algorithmic_bytes_per_launch", "avg_launch_us", "traffic", "frac_dram",
-                                               "equivalent_gbs", "bytes_model", "peak_source")}
+                                               "equivalent_gbs", "bytes_model", "peak_source", "frac_read")}
+    h["roofline"]["read_stream_gbs"] = full.get("read_stream_gbs")
     if roof.get("traffic_stale"):
         h["roofline"]["traffic_stale"] = True
     h["roofline"]["also"] = picked[:10]
@@ -950,6 +978,7 @@ def run_ours(args):
     if rank == 0:
         also = []
         name = "%s-%d" % (PREC_NAME[prec], recon)
+        read_gbs = read_stream_gbs(torch)                 # sets the `frac_read` of every roofline entry below
         # ---- roofline of the step's dominant kernel ------------------------------------------------
         if persistent:
             # the whole solve is ONE kernel (stag_cg_persist.cuh): that kernel is the step.  `achieved` uses the
@@ -1013,6 +1042,7 @@ def run_ours(args):
                      % (2 * nshift + 4, wset / 1e6, "exceeds" if wset > l2_bytes else "FITS in", l2_bytes / 1e6,
                         "; no flush between steps" if wset > l2_bytes else
                         ": an L2-resident run, not held to the HBM roofline"),
+               "read_stream_gbs": read_gbs,
                "dslash_gflops_through_solve": value,
                "dslash_gflops_standalone": dslash[name]["gflops"],
                "cg_s_per_solve": secs / args.steps,

@@ -35,6 +35,8 @@
 //   * oracle_partial_fraction — y = residue0*b + sum_i residues[i]*x_i.
 //
 // No blocking, fusion, tables or reordering: loops over sites, arithmetic neighbours.
+// The threaded mode (oracle_set_threads(k > 1): OpenMP over sites, chunk-ordered deterministic
+// reductions) is pinned by P11: bit-equal to one thread for k = 2, 5, 8.
 // Every function here is pinned (no "parity unpinned" function); what is unpinned against
 // the PAPER is only the particular equivalent eta / axis convention (readings A2, A4).
 

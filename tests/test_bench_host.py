@@ -159,7 +159,8 @@ def test_headline_line_is_short_strict_json_with_the_contract_keys():
     assert 1 <= len(r["also"]) <= 10
     assert [(e["workload"], e["tag"]) for e in r["also"]] == list(bench.HEADLINE_ALSO)
     for e in r["also"]:
-        assert set(e) <= {"workload", "tag", "kernel", "frac", "avg_launch_us", "traffic", "frac_dram", "traffic_stale"}
+        assert set(e) <= {"workload", "tag", "kernel", "frac", "frac_read", "avg_launch_us", "traffic", "frac_dram",
+                          "traffic_stale"}
     assert h["c5"]["timed_solves"] == 3 and h["c5"]["gflops_through_solve"] is None      # the NaN became null
     assert abs(h["c5"]["frac"] - 1.032) < 1e-6
     assert h["cpu_baseline"]["cores"] == 1 and h["cpu_baseline"]["all_cores"]["cores"] == 32
